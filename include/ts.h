@@ -1,0 +1,209 @@
+/*
+ * ts.h -- C ABI of libts: batched pair-potential MD / FIRE on one B200 (sm_100a).
+ *
+ * The boundary named by BASELINE.json:north_star ("ts_state_create, ts_build_neighbors,
+ * ts_compute_forces, ts_md_step, ts_fire_step") and laid out in SURVEY.md section 8(b).  The
+ * operation is the paper's batched simulation: "The attributes of individual systems, such as
+ * positions and momenta, are concatenated into a single SimState object ... concatenates atom-wise
+ * ... and stacks batch-wise attributes (unit cell, stress tensor, etc.)" (section 3),
+ * a model call that returns "energies, forces, and stress" (section 2) for the
+ * classical potentials "Lennard-Jones, Morse, soft-sphere" (Abstract), advanced by
+ * "molecular dynamics integrators" / "structural relaxation optimizers", with the
+ * convergence check and swap of the InFlightAutobatcher (section 3).  The paper prints
+ * no formula; the formulas are O1..O6 of SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Conventions
+ *  - Plain C types only.  "device" = pointer into CUDA device memory of the current device,
+ *    "host" = ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL = default).
+ *  - Ownership: the CALLER owns every device array in ts_state_desc and the workspace blob; the
+ *    library borrows them until ts_state_destroy and allocates no device memory itself.  The
+ *    library owns only the host-side ts_state.  Outputs are written in place.
+ *  - Layout at the boundary: [N,3] row-major positions / velocities / forces, [N] per-atom scalars,
+ *    [S,3,3] cells whose ROWS are lattice vectors (x = f . h, all three directions periodic),
+ *    per-atom system_idx non-decreasing 0..S-1.  All floating arrays of one state share `dtype`
+ *    except energy / virial / kinetic, which are always float64.
+ *  - Stored positions are never wrapped by the library.
+ *  - Calls are asynchronous on `stream` unless stated.  A ts_state is not thread-safe.
+ *  - Errors: argument errors return immediately (nothing enqueued).  Conditions found on the device
+ *    (neighbour capacity overflow, image shift out of range, non-finite force, bad cell) set sticky
+ *    bits in a device status word; ts_poll reports them and every later stepping call returns
+ *    TS_ERR_STICKY until ts_clear_error.  On overflow nothing is written past capacity.
+ *  - No CPU fallback exists: every entry point needs a CUDA device.
+ */
+#ifndef TS_H
+#define TS_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_state ts_state;   /* opaque, host-side, owned by the library */
+typedef int32_t ts_status;
+
+enum {
+    TS_OK = 0,
+    TS_ERR_INVALID_ARG = 1,
+    TS_ERR_CUDA = 2,
+    TS_ERR_WORKSPACE_TOO_SMALL = 3,
+    TS_ERR_NBR_OVERFLOW = 4,
+    TS_ERR_STALE_NBR = 5,
+    TS_ERR_NONFINITE = 6,
+    TS_ERR_UNSUPPORTED = 7,
+    TS_ERR_STICKY = 8
+};
+
+/* bits of ts_report.flags (device status word) */
+enum {
+    TS_FLAG_NBR_OVERFLOW = 1u,   /* neighbour list larger than the workspace capacity             */
+    TS_FLAG_SHIFT_RANGE = 2u,    /* an image shift left [-16,15] (atom > 15 cells from its image)  */
+    TS_FLAG_NONFINITE = 4u,      /* a non-finite force was produced                                */
+    TS_FLAG_BAD_CELL = 8u        /* singular cell, or a stencil wider than 31 bins                 */
+};
+
+typedef enum { TS_F32 = 0, TS_F64 = 1 } ts_dtype;
+typedef enum { TS_LJ = 0, TS_MORSE = 1, TS_SOFT_SPHERE = 2 } ts_pot_kind;
+enum { TS_WANT_ENERGY = 1u, TS_WANT_VIRIAL = 2u };
+enum { TS_NVE = 0, TS_BAOAB = 1 };
+enum { TS_FIRE_FRESH = 0, TS_FIRE_RUNNING = 1, TS_FIRE_CONVERGED = 2, TS_FIRE_FAILED = 3 };
+
+/* Units: a = F / (m * mass_conv).  metal: mass_conv = 103.64269652680505
+ * (eV fs^2 / (amu A^2)), kB = 8.617333262145179e-5 eV/K; reduced units: 1, 1.                     */
+typedef struct { double mass_conv; double kB; } ts_units;
+
+/* Pair potential.  HOST tables [n_types*n_types], entry (ti*n_types + tj); copied at
+ * create.  LJ:    V = 4 p0 [(p1/r)^12 - (p1/r)^6]                      p0 = eps, p1 = sigma
+ * Morse:          V = p0 [(1 - exp(-p1 (r - p2)))^2 - 1]               p0 = D, p1 = alpha, p2 = r0
+ * soft sphere:    V = (p0/p2) (1 - r/p1)^p2 for r < p1, else 0         p0 = eps, p1 = sigma, p2 = exponent
+ * Pairs with r >= rc contribute exactly 0 (strict r^2 < rc^2).  shift_energy: V <- V - V(rc).     */
+typedef struct {
+    int32_t kind;            /* ts_pot_kind */
+    int32_t n_types;
+    const double *p0, *p1, *p2, *rc;
+    int32_t shift_energy;
+} ts_potential;
+
+/* The batch.  All pointers device unless NULL is allowed.                           */
+typedef struct {
+    int64_t n_atoms;         /* N >= 1 */
+    int32_t n_systems;       /* S >= 1 */
+    int32_t dtype;           /* ts_dtype of pos, vel, force, mass, cell */
+    ts_units units;
+    void *pos;               /* [N,3] in/out */
+    void *vel;               /* [N,3] in/out */
+    void *force;             /* [N,3] out    */
+    const void *mass;        /* [N]   in     */
+    const int32_t *type;     /* [N]   in, 0..n_types-1 */
+    const int32_t *system_idx; /* [N] in, non-decreasing; every system has >= 1 and <= 131072 atoms */
+    const void *cell;        /* [S,3,3] in, rows = lattice vectors */
+    double *energy;          /* [S]     out, potential energy E_s (float64) */
+    double *virial;          /* [S,3,3] out, W_s = -dE/dstrain (float64); stress = -W/V */
+    double *kinetic;         /* [S]     out, KE_s = 1/2 sum m mass_conv v^2 (float64) */
+    const uint32_t *sys_uid; /* [S] persistent ids for the Philox counter (R18); NULL -> 0..S-1 */
+} ts_state_desc;
+
+/* skin: Verlet skin (list radius = max rc + skin; rebuild when an atom moved > skin/2).
+ * slack: capacity factor on the estimated pair count (>= 1; 0 -> 1.25).                           */
+typedef struct { double skin; double slack; } ts_nbr_params;
+
+/* integrator TS_NVE: velocity Verlet.  TS_BAOAB: Langevin B A O A B (O4) with one
+ * Philox4x32-10 block per atom per step, key = seed, counter = (local atom index, sys_uid,
+ * step lo, step hi) (O5).  friction in 1/time, temperature in K (uses units.kB).                  */
+typedef struct { int32_t integrator; double dt, temperature, friction; uint64_t seed; } ts_md_params;
+
+/* FIRE, MD form: Bitzek et al., PRL 97, 170201 (2006).                                */
+typedef struct {
+    double dt_start, dt_max, f_inc, f_dec, alpha_start, f_alpha, f_max;
+    int32_t n_min, max_steps;
+} ts_fire_params;
+
+typedef struct {
+    uint32_t flags;          /* TS_FLAG_* sticky bits */
+    int32_t n_rebuilds;      /* neighbour builds since create */
+    int64_t nnz;             /* directed pairs in the current list */
+    int64_t nnz_capacity;
+    int64_t steps_done;      /* MD/FIRE steps enqueued since create */
+    int32_t n_converged;     /* systems with FIRE status converged */
+    int32_t n_failed;        /* systems that hit max_steps */
+    int32_t max_neighbors;   /* longest row of the current list */
+    int32_t list_valid;
+} ts_report;
+
+/* Bytes of workspace ts_state_create needs for this batch (the memory-estimate primitive, SURVEY
+ * a9).  Reads the cells from the device (synchronises).                                           */
+ts_status ts_workspace_bytes(const ts_state_desc *desc, const ts_potential *pot,
+                             const ts_nbr_params *nbr, size_t *out_bytes);
+
+/* Host-only variant of the same estimate for one system of n_atoms in volume `volume`: bytes of
+ * workspace plus boundary arrays that system adds to a batch.  No device needed.                  */
+ts_status ts_estimate_system_bytes(int64_t n_atoms, double volume, double r_list, double slack,
+                                   int32_t dtype, size_t *out_bytes);
+
+/* Create a state over caller-owned arrays.  workspace: device, 256-byte aligned, workspace_bytes >=
+ * ts_workspace_bytes.  Validates system_idx (synchronises once).  Imports pos/vel.               */
+ts_status ts_state_create(const ts_state_desc *desc, const ts_potential *pot,
+                          const ts_nbr_params *nbr, void *workspace, size_t workspace_bytes,
+                          ts_state **out);
+ts_status ts_state_destroy(ts_state *st);
+
+/* Cell-list neighbour build from the current desc.pos: binning + counting sort by
+ * (system, cell), count -> scan -> capacity check -> fill of the CSR list at radius max rc + skin. */
+ts_status ts_build_neighbors(ts_state *st, void *stream);
+
+/* Forces (always), energy / virial when asked from the current desc.pos; rebuilds
+ * the list first if it is missing or an atom moved more than skin/2 since the last build.        */
+ts_status ts_compute_forces(ts_state *st, uint32_t want, void *stream);
+
+/* n_steps of MD entirely on the device, skin checks and rebuilds included.  On
+ * return of the enqueued work: pos, vel at t + n dt, force = F(pos), energy, kinetic (and virial if
+ * want has TS_WANT_VIRIAL) of the final state (R16).                                              */
+ts_status ts_md_step(ts_state *st, const ts_md_params *p, int32_t n_steps, uint32_t want,
+                     void *stream);
+
+/* Up to n_steps of FIRE on every system that is not frozen.  Fresh systems are
+ * initialised (v = 0, dt_start, alpha_start) and checked for convergence with 0 steps.  Converged
+ * and failed systems are left bit-unchanged.                                                      */
+ts_status ts_fire_step(ts_state *st, const ts_fire_params *p, int32_t n_steps, void *stream);
+
+/* Synchronises `stream` and reports.  Returns TS_OK even when flags are set (read out->flags).    */
+ts_status ts_poll(ts_state *st, ts_report *out, void *stream);
+
+/* Synchronising read of the per-system FIRE status into HOST arrays (any may be NULL):
+ * mask[s] = 1 when converged; status[s] = TS_FIRE_*; fire_steps[s] = steps taken so far.          */
+ts_status ts_converged_mask(ts_state *st, uint8_t *mask, int32_t *status, int32_t *fire_steps,
+                            void *stream);
+
+/* In-flight swap: replace the systems in `slots` (HOST, n entries) by the
+ * n systems of `fresh` (device arrays pos, vel, mass, type, cell, sys_uid; system k of fresh must
+ * have exactly as many atoms as slot slots[k]).  Their FIRE state becomes fresh, their step
+ * counter 0, and the neighbour list is marked stale.                                              */
+ts_status ts_swap_systems(ts_state *st, const int32_t *slots, int32_t n, const ts_state_desc *fresh,
+                          void *stream);
+
+/* Synchronising export of the current list to HOST arrays (test / graph export): off [N+1], and
+ * for each directed pair its GLOBAL neighbour index j and image shift S (relative to the stored
+ * positions, R6).  cap = capacity of j / shift in pairs; TS_ERR_WORKSPACE_TOO_SMALL if nnz > cap. */
+ts_status ts_get_neighbors(ts_state *st, int64_t *off, int32_t *j, int8_t *shift, int64_t cap,
+                           void *stream);
+
+/* Per-system step counters used by the Philox counter (R18): HOST [S] in / out.  Synchronising.   */
+ts_status ts_set_system_steps(ts_state *st, const uint64_t *steps, void *stream);
+ts_status ts_get_system_steps(ts_state *st, uint64_t *steps, void *stream);
+
+/* Select the stepping engine: 0 = general multi-kernel path (any system size), 1 = system-resident
+ * path (whole systems held in shared memory across steps) where the batch allows it, falling back
+ * to 0 otherwise.  Default 1.  Results obey the same tolerances either way.                       */
+ts_status ts_set_engine(ts_state *st, int32_t engine);
+
+/* Number of kernel launches enqueued by this state since create (for bench accounting).           */
+int64_t ts_launch_count(const ts_state *st);
+
+ts_status ts_clear_error(ts_state *st, void *stream);
+const char *ts_status_string(ts_status s);
+const char *ts_last_error(const ts_state *st);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TS_H */
