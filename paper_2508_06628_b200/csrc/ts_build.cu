@@ -1,0 +1,324 @@
+/*
+ * ts_build.cu -- binned cell-list neighbour build (readings R5..R9, R27).
+ *
+ * Pipeline (all kernels early-exit unless status->need_rebuild is set, so the whole build can sit
+ * in the stream every step without a host round trip):
+ *   k_build_begin : zero the per-cell counters
+ *   k_bin         : f = x . h^-1 (fp64), wrap = floor(f), bin id, rank in cell (atomic counter)
+ *   k_cellscan    : per-system exclusive scan of the cell counters (block per system; the key
+ *                   space of system s is [sysoff[s]+s, sysoff[s+1]+s] so no global scan exists)
+ *   k_scatter     : counting-sort scatter of wrapped fp64 coordinates; x_ref and pos4 refresh
+ *   k_nbr<0>      : warp-cooperative scan of the (2D+1)^3 extended-bin stencil, COUNT
+ *   k_nbrscan     : per-system exclusive scan of the counts + capacity check (overflow flag)
+ *   k_nbr<1>      : same scan, FILL of the CSR rows (skipped for overflowed systems)
+ * The cutoff test is strict r^2 < r_list^2 in fp64 on the promoted coordinates (R9, R27).
+ */
+#include "ts_internal.cuh"
+
+template <typename T>
+__global__ void k_geometry(DevState d, const int *slots, int count)
+{
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= count) return;
+    int s = slots ? slots[t] : t;
+    const T *c = (const T *)d.cell + 9 * (size_t)s;
+    SysGeom g;
+    for (int k = 0; k < 9; ++k) g.h[k] = (double)c[k];
+    const double *h = g.h;
+    double c00 = h[4] * h[8] - h[5] * h[7];
+    double c01 = h[5] * h[6] - h[3] * h[8];
+    double c02 = h[3] * h[7] - h[4] * h[6];
+    double det = h[0] * c00 + h[1] * c01 + h[2] * c02;
+    g.bad = !(fabs(det) > 0.0);
+    double id = g.bad ? 0.0 : 1.0 / det;
+    g.hinv[0] = c00 * id;
+    g.hinv[1] = (h[2] * h[7] - h[1] * h[8]) * id;
+    g.hinv[2] = (h[1] * h[5] - h[2] * h[4]) * id;
+    g.hinv[3] = c01 * id;
+    g.hinv[4] = (h[0] * h[8] - h[2] * h[6]) * id;
+    g.hinv[5] = (h[2] * h[3] - h[0] * h[5]) * id;
+    g.hinv[6] = c02 * id;
+    g.hinv[7] = (h[1] * h[6] - h[0] * h[7]) * id;
+    g.hinv[8] = (h[0] * h[4] - h[1] * h[3]) * id;
+    g.vol = fabs(det);
+    int ns = d.sysoff[s + 1] - d.sysoff[s];
+    for (int k = 0; k < 3; ++k) {
+        double n2 = g.hinv[k] * g.hinv[k] + g.hinv[3 + k] * g.hinv[3 + k] + g.hinv[6 + k] * g.hinv[6 + k];
+        g.hperp[k] = g.bad ? 1.0 : 1.0 / sqrt(n2);
+        double q = g.hperp[k] / d.r_list;
+        g.nb[k] = q >= 2.0 ? (q < 1024.0 ? (int)floor(q) : 1024) : 1;
+    }
+    /* never more cells than atoms: the per-system key space has ns + 1 slots */
+    while ((long long)g.nb[0] * g.nb[1] * g.nb[2] > (long long)(ns > 1 ? ns : 1)) {
+        int m = (g.nb[0] >= g.nb[1] && g.nb[0] >= g.nb[2]) ? 0 : (g.nb[1] >= g.nb[2] ? 1 : 2);
+        g.nb[m] -= 1;
+    }
+    g.ncell = g.nb[0] * g.nb[1] * g.nb[2];
+    for (int k = 0; k < 3; ++k) {
+        double w = d.r_list * (double)g.nb[k] / g.hperp[k];
+        int D = (int)ceil(w * (1.0 + 1e-12));
+        if (D < 1) D = 1;
+        if (D > 15) { D = 15; g.bad = 1; }
+        g.D[k] = D;
+    }
+    if (g.bad) atomicOr(&d.status->flags, TS_FLAG_BAD_CELL);
+    d.geom[s] = g;
+    T *hT = (T *)d.hT + 9 * (size_t)s;
+    for (int k = 0; k < 9; ++k) hT[k] = c[k];
+}
+
+__global__ void k_build_begin(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    long long n = d.N + d.S + 1;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        d.cell_count[i] = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        d.status->nnz = 0ull;
+        d.status->max_nbr = 0u;
+        d.status->list_valid = 1u;
+    }
+}
+
+__global__ void k_build_end(DevState d) { d.status->need_rebuild = 0u; }
+
+template <typename T>
+__global__ void k_bin(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    int s = d.sysidx[i];
+    const SysGeom &g = d.geom[s];
+    const T *x = (const T *)d.pos + 3 * i;
+    double x0 = (double)x[0], x1 = (double)x[1], x2 = (double)x[2];
+    int c[3], w[3];
+    bool range = false;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double f = x0 * g.hinv[k] + x1 * g.hinv[3 + k] + x2 * g.hinv[6 + k];
+        double fl = floor(f);
+        double fw = f - fl;
+        int nb = g.nb[k];
+        int ck = (int)(fw * (double)nb);
+        c[k] = ck < 0 ? 0 : (ck >= nb ? nb - 1 : ck);
+        if (!(fabs(fl) <= 100.0)) { range = true; fl = 0.0; }
+        w[k] = (int)fl;
+    }
+    if (range) atomicOr(&d.status->flags, TS_FLAG_SHIFT_RANGE);
+    int cid = ts_cell_base(d.sysoff, s) + (c[0] * g.nb[1] + c[1]) * g.nb[2] + c[2];
+    d.atom_cell[i] = cid;
+    d.atom_rank[i] = atomicAdd(&d.cell_count[cid], 1);
+    d.atom_wrap[i] = ts_pack_wrap(w[0], w[1], w[2]);
+}
+
+/* Exclusive block scan helper: returns the exclusive prefix of v, total in *tot (all threads). */
+template <typename V>
+__device__ __forceinline__ V block_excl_scan(V v, V *sh /* [33] */, V *tot)
+{
+    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    V inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        V u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+    }
+    __syncthreads();
+    if (lane == 31) sh[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        V w = lane < nw ? sh[lane] : (V)0;
+        V winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            V u = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += u;
+        }
+        if (lane < nw) sh[lane] = winc - w;
+        if (lane == 31) sh[32] = winc;
+    }
+    __syncthreads();
+    *tot = sh[32];
+    return inc - v + sh[wid];
+}
+
+__global__ void k_cellscan(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    __shared__ int sh[33];
+    int s = blockIdx.x;
+    int base = ts_cell_base(d.sysoff, s);
+    int nc = d.geom[s].ncell;
+    int run = d.sysoff[s];
+    for (int c0 = 0; c0 < nc; c0 += blockDim.x) {
+        int c = c0 + threadIdx.x;
+        int v = c < nc ? d.cell_count[base + c] : 0;
+        int tot;
+        int ex = block_excl_scan<int>(v, sh, &tot);
+        if (c < nc) d.cell_start[base + c] = run + ex;
+        run += tot;
+    }
+    if (threadIdx.x == 0) {
+        d.cell_start[base + nc] = run;
+        if (s == 0) d.status->n_rebuilds += 1;
+    }
+}
+
+template <typename T>
+__global__ void k_scatter(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    int s = d.sysidx[i];
+    const SysGeom &g = d.geom[s];
+    const T *x = (const T *)d.pos + 3 * i;
+    T xs0 = x[0], xs1 = x[1], xs2 = x[2];
+    int w0, w1, w2;
+    ts_unpack_wrap(d.atom_wrap[i], w0, w1, w2);
+    double xw0 = (double)xs0 - ((double)w0 * g.h[0] + (double)w1 * g.h[3] + (double)w2 * g.h[6]);
+    double xw1 = (double)xs1 - ((double)w0 * g.h[1] + (double)w1 * g.h[4] + (double)w2 * g.h[7]);
+    double xw2 = (double)xs2 - ((double)w0 * g.h[2] + (double)w1 * g.h[5] + (double)w2 * g.h[8]);
+    int p = d.cell_start[d.atom_cell[i]] + d.atom_rank[i];
+    int li = (int)(i - d.sysoff[s]);
+    d.spos[p] = make_double4(xw0, xw1, xw2, __longlong_as_double((long long)li));
+    T *xr = (T *)d.xref + 3 * i;
+    xr[0] = xs0; xr[1] = xs1; xr[2] = xs2;
+    typedef typename Vec4<T>::type V4;
+    V4 q;
+    q.x = (T)xw0; q.y = (T)xw1; q.z = (T)xw2;
+    int ty = d.type[i];
+    if (sizeof(T) == 4) q.w = (T)__int_as_float(ty); else q.w = (T)__longlong_as_double((long long)ty);
+    ((V4 *)d.pos4)[i] = q;
+}
+
+__device__ __forceinline__ int floordiv(int a, int n) { int q = a / n; return (a % n < 0) ? q - 1 : q; }
+
+/* One warp per sorted slot p.  Lanes stride over the atoms of each stencil cell. */
+template <int FILL>
+__global__ void k_nbr(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    long long p = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (p >= d.N) return;
+    int s = d.sysidx[p];                 /* sorted slots of a system occupy the system's own range */
+    if (FILL && d.nbr_len[s] < 0) return;
+    const SysGeom &g = d.geom[s];
+    int a0 = d.sysoff[s];
+    int base = a0 + s;
+    double4 me = d.spos[p];
+    int li = (int)__double_as_longlong(me.w);
+    int lin = d.atom_cell[a0 + li] - base;
+    int nb0 = g.nb[0], nb1 = g.nb[1], nb2 = g.nb[2];
+    int c2 = lin % nb2, c1 = (lin / nb2) % nb1, c0 = lin / (nb2 * nb1);
+    int D0 = g.D[0], D1 = g.D[1], D2 = g.D[2];
+    double R2 = d.r_list2;
+    int cnt = 0;
+    long long off = FILL ? d.nbr_off[a0 + li] : 0;
+    unsigned lt = (1u << lane) - 1u;
+    for (int e0 = c0 - D0; e0 <= c0 + D0; ++e0) {
+        int s0 = floordiv(e0, nb0), b0 = e0 - s0 * nb0;
+        for (int e1 = c1 - D1; e1 <= c1 + D1; ++e1) {
+            int s1 = floordiv(e1, nb1), b1 = e1 - s1 * nb1;
+            for (int e2 = c2 - D2; e2 <= c2 + D2; ++e2) {
+                int s2 = floordiv(e2, nb2), b2 = e2 - s2 * nb2;
+                int cell = base + (b0 * nb1 + b1) * nb2 + b2;
+                int q0 = d.cell_start[cell], q1 = d.cell_start[cell + 1];
+                if (q0 == q1) continue;
+                double sx = (double)s0 * g.h[0] + (double)s1 * g.h[3] + (double)s2 * g.h[6] - me.x;
+                double sy = (double)s0 * g.h[1] + (double)s1 * g.h[4] + (double)s2 * g.h[7] - me.y;
+                double sz = (double)s0 * g.h[2] + (double)s1 * g.h[5] + (double)s2 * g.h[8] - me.z;
+                bool home = (s0 == 0) & (s1 == 0) & (s2 == 0);
+                for (int q = q0; q < q1; q += 32) {
+                    int qq = q + lane;
+                    bool ok = false;
+                    int lj = 0;
+                    if (qq < q1) {
+                        double4 c = d.spos[qq];
+                        double rx = c.x + sx, ry = c.y + sy, rz = c.z + sz;
+                        double r2 = rx * rx + ry * ry + rz * rz;
+                        lj = (int)__double_as_longlong(c.w);
+                        ok = (r2 < R2) && !(home && qq == (int)p);
+                    }
+                    unsigned m = __ballot_sync(0xffffffffu, ok);
+                    if (FILL && ok) d.nbr[off + cnt + __popc(m & lt)] = ts_pack_nbr(lj, s0, s1, s2);
+                    cnt += __popc(m);
+                }
+            }
+        }
+    }
+    if (!FILL && lane == 0) d.nbr_cnt[a0 + li] = cnt;
+}
+
+__global__ void k_nbrscan(DevState d)
+{
+    if (!d.status->need_rebuild) return;
+    __shared__ long long sh[33];
+    __shared__ int shm[32];
+    int s = blockIdx.x;
+    int a0 = d.sysoff[s], a1 = d.sysoff[s + 1];
+    long long base = d.nbr_base[s], cap = d.nbr_base[s + 1] - base;
+    long long run = 0;
+    int mx = 0;
+    for (int i0 = a0; i0 < a1; i0 += blockDim.x) {
+        int i = i0 + threadIdx.x;
+        long long v = i < a1 ? (long long)d.nbr_cnt[i] : 0;
+        mx = max(mx, (int)v);
+        long long tot;
+        long long ex = block_excl_scan<long long>(v, sh, &tot);
+        if (i < a1) d.nbr_off[i] = base + run + ex;
+        run += tot;
+    }
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0) shm[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mx = max(mx, shm[w]);
+        atomicMax(&d.status->max_nbr, (unsigned)mx);
+        atomicAdd(&d.status->nnz, (unsigned long long)run);
+        if (run > cap) {
+            d.nbr_len[s] = -1;
+            atomicOr(&d.status->flags, TS_FLAG_NBR_OVERFLOW);
+            d.status->list_valid = 0u;
+        } else {
+            d.nbr_len[s] = run;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ host launchers */
+void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, cudaStream_t q)
+{
+    (void)s_first;
+    int nb = (s_count + 127) / 128;
+    if (st->d.dtype == TS_F32) k_geometry<float><<<nb, 128, 0, q>>>(st->d, slots, s_count);
+    else k_geometry<double><<<nb, 128, 0, q>>>(st->d, slots, s_count);
+    st->launches += 1;
+}
+
+__global__ void k_force_rebuild(DevState d)
+{
+    d.status->need_rebuild = 1u;
+}
+
+void launch_build(ts_state *st, bool force, cudaStream_t q)
+{
+    const DevState &d = st->d;
+    if (force) { k_force_rebuild<<<1, 1, 0, q>>>(d); st->launches += 1; }
+    long long n = d.N + d.S + 1;
+    int tb = 256;
+    int nbz = (int)((n + tb - 1) / tb); if (nbz > 148 * 8) nbz = 148 * 8;
+    int nba = (int)((d.N + tb - 1) / tb);
+    long long nwarp_blocks = (d.N * 32 + tb - 1) / tb;
+    k_build_begin<<<nbz, tb, 0, q>>>(d);
+    if (d.dtype == TS_F32) k_bin<float><<<nba, tb, 0, q>>>(d); else k_bin<double><<<nba, tb, 0, q>>>(d);
+    k_cellscan<<<d.S, 256, 0, q>>>(d);
+    if (d.dtype == TS_F32) k_scatter<float><<<nba, tb, 0, q>>>(d); else k_scatter<double><<<nba, tb, 0, q>>>(d);
+    k_nbr<0><<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
+    k_nbrscan<<<d.S, 256, 0, q>>>(d);
+    k_nbr<1><<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
+    k_build_end<<<1, 1, 0, q>>>(d);
+    st->launches += 8;
+    st->list_built = true;
+}

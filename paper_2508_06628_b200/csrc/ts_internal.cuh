@@ -1,0 +1,181 @@
+/*
+ * ts_internal.cuh -- structures shared by the translation units of libts (CUDA path only; the
+ * oracle under oracle/ shares nothing with this tree).
+ *
+ * Data layout in HBM:
+ *   boundary arrays (caller-owned): pos/vel/force [N,3], mass [N], type [N], system_idx [N],
+ *                                   cell [S,3,3], energy [S], virial [S,9], kinetic [S]
+ *   workspace (caller-owned blob, carved by ts_layout):
+ *     per system : sysoff, SysGeom (fp64 cell, inverse, heights, bin grid, stencil half-widths),
+ *                  hT (cell in the state dtype), nbr_base / nbr_len (CSR segment of the system),
+ *                  FIRE scalars, step counter
+ *     per atom   : pos4 (x~,y~,z~,type) gather array, spos (bin-sorted wrapped fp64 coordinates +
+ *                  local index), xref (positions at the last build), cell id / rank / wrap,
+ *                  nbr_cnt, nbr_off
+ *     per pair   : packed uint32 neighbour entry = local j (17 bits) | 3 x 5-bit biased shift
+ */
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "ts.h"
+
+#define TS_MAX_TYPES 8
+#define TS_J_BITS 17
+#define TS_J_MASK 0x1FFFFu
+#define TS_MAX_SYS_ATOMS (1 << TS_J_BITS)
+
+struct SysGeom {
+    double h[9];      /* rows = lattice vectors                         */
+    double hinv[9];   /* f_k = sum_b x_b hinv[3b+k]                      */
+    double hperp[3];  /* distance between lattice planes k               */
+    double vol;
+    int nb[3];        /* bins per axis                                   */
+    int D[3];         /* stencil half-width in bins (R8)                 */
+    int ncell;
+    int bad;
+};
+
+template <typename T>
+struct PotEntry {
+    T p0, p1, p2, rc2, vshift;
+    T c0, c1, c2;     /* precomputed: LJ 4 eps s^12, 4 eps s^6 ; Morse 2 D alpha ; soft eps/alpha, eps/sigma, 1/sigma */
+};
+
+struct DevStatus {
+    unsigned int flags;         /* TS_FLAG_* sticky                                  */
+    unsigned int need_rebuild;  /* set by the skin check, cleared after a build      */
+    unsigned int n_rebuilds;
+    unsigned int max_nbr;
+    unsigned long long nnz;
+    unsigned int list_valid;
+    unsigned int pad;
+};
+
+/* Everything a kernel needs, passed by value (well under the 4 KB parameter limit). */
+struct DevState {
+    long long N;
+    int S;
+    int dtype;
+    int kind, n_types, shift_energy;
+    double mass_conv, kB;
+    double r_list, r_list2, half_skin2;
+    /* boundary */
+    void *pos, *vel, *force;
+    const void *mass;
+    const int *type;
+    const int *sysidx;
+    const void *cell;
+    double *energy, *virial, *kinetic;
+    const unsigned int *uid;
+    /* workspace: per system */
+    int *sysoff;                 /* [S+1]                              */
+    SysGeom *geom;               /* [S]                                */
+    void *hT;                    /* [S,9] cell in state dtype          */
+    long long *nbr_base;         /* [S+1] first pair slot of a system  */
+    long long *nbr_len;          /* [S]  pairs in use, -1 = overflow   */
+    double *f_dt, *f_alpha;      /* [S] FIRE                           */
+    int *f_npos, *f_nsteps, *f_status;
+    double *f_acc;               /* [S,4] fmax2, P, vv, ff             */
+    int *sys_active;             /* [S] 1 = atoms of the system move   */
+    unsigned long long *sys_step;/* [S] per-system step counter (R18)  */
+    unsigned int *uid_own;       /* [S] persistent ids (copy or iota)  */
+    /* workspace: per atom */
+    void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
+    double4 *spos;               /* [N] sorted wrapped coords + local idx */
+    void *xref;                  /* [N,3] state dtype                  */
+    int *cell_count, *cell_start;/* [N+S+1]                            */
+    int *atom_cell, *atom_rank, *atom_wrap; /* [N]                     */
+    int *nbr_cnt;                /* [N]                                */
+    long long *nbr_off;          /* [N]                                */
+    /* workspace: per pair */
+    unsigned int *nbr;           /* [cap]                              */
+    long long nbr_cap;
+    void *pot;                   /* PotEntry<T> [n_types^2]            */
+    DevStatus *status;
+    int *scratch;                /* small upload area (swap lists)     */
+};
+
+struct ts_state {
+    DevState d;
+    ts_state_desc desc;
+    ts_nbr_params nbr;
+    int *h_sysoff;               /* host copy [S+1]                    */
+    bool list_built;             /* a build has been enqueued and no swap since */
+    bool forces_current;
+    int engine;
+    long long launches;
+    long long steps_done;
+    unsigned int seen_flags;     /* last flags seen by ts_poll         */
+    char err[256];
+};
+
+/* ------------------------------------------------------------------ workspace carving */
+struct TsLayout {
+    size_t total;
+    size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
+        sys_active, sys_step, uid_own, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
+};
+TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);
+
+/* ------------------------------------------------------------------ launchers (host) */
+#define TS_CUDA_OK(st, call)                                                              \
+    do {                                                                                  \
+        cudaError_t e__ = (call);                                                         \
+        if (e__ != cudaSuccess) {                                                         \
+            ts_set_error((st), "CUDA error %s at %s:%d", cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return TS_ERR_CUDA;                                                           \
+        }                                                                                 \
+    } while (0)
+void ts_set_error(ts_state *st, const char *fmt, ...);
+
+/* ts_build.cu */
+void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, cudaStream_t q);
+void launch_build(ts_state *st, bool force, cudaStream_t q);
+/* ts_pair.cu */
+void launch_pair(ts_state *st, unsigned want, bool masked, cudaStream_t q);
+/* ts_integrate.cu */
+struct MdConst { int integrator; double dt, hdt, c1, c2, kT; unsigned int key0, key1; };
+void launch_import(ts_state *st, cudaStream_t q);   /* pos -> pos4 + skin check */
+void launch_md_pre(ts_state *st, const MdConst &c, cudaStream_t q);
+void launch_md_post(ts_state *st, const MdConst &c, bool want_ke, cudaStream_t q);
+void launch_kinetic(ts_state *st, cudaStream_t q);
+void launch_fire_init(ts_state *st, const ts_fire_params &p, cudaStream_t q);
+void launch_fire_check0(ts_state *st, const ts_fire_params &p, cudaStream_t q);
+void launch_fire_pre(ts_state *st, const ts_fire_params &p, cudaStream_t q);
+void launch_fire_post(ts_state *st, const ts_fire_params &p, cudaStream_t q);
+void launch_fire_count(ts_state *st, cudaStream_t q);
+void launch_swap(ts_state *st, int n, const ts_state_desc *fresh, cudaStream_t q);
+/* ts_resident.cu */
+bool resident_supported(const ts_state *st);
+ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q);
+
+/* ------------------------------------------------------------------ device helpers */
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { typedef float4 type; };
+template <> struct Vec4<double> { typedef double4 type; };
+
+__device__ __forceinline__ int ts_cell_base(const int *sysoff, int s) { return sysoff[s] + s; }
+
+__device__ __forceinline__ unsigned int ts_pack_nbr(int j, int s0, int s1, int s2)
+{
+    return (unsigned)j | ((unsigned)(s0 + 16) << 17) | ((unsigned)(s1 + 16) << 22) | ((unsigned)(s2 + 16) << 27);
+}
+__device__ __forceinline__ void ts_unpack_shift(unsigned int e, int &s0, int &s1, int &s2)
+{
+    s0 = (int)((e >> 17) & 31u) - 16;
+    s1 = (int)((e >> 22) & 31u) - 16;
+    s2 = (int)(e >> 27) - 16;
+}
+__device__ __forceinline__ int ts_pack_wrap(int w0, int w1, int w2)
+{
+    return (w0 & 0xff) | ((w1 & 0xff) << 8) | ((w2 & 0xff) << 16);
+}
+__device__ __forceinline__ void ts_unpack_wrap(int p, int &w0, int &w1, int &w2)
+{
+    w0 = (int)(signed char)(p & 0xff);
+    w1 = (int)(signed char)((p >> 8) & 0xff);
+    w2 = (int)(signed char)((p >> 16) & 0xff);
+}

@@ -1,0 +1,209 @@
+/*
+ * ts_pair.cu -- pair-potential kernel over the CSR Verlet list.
+ *
+ *   F_i = sum_{(i,j,S)} V'(r) r/|r|,  r = x~_j - x~_i + S.h      (r points i -> j)
+ *   E_s = 1/2 sum V(r) (shifted by V(rc) when shift_energy),  W_s = -1/2 sum V'(r) (r (x) r)/r
+ * Pairs with r^2 >= rc^2 that sit in the Verlet shell contribute exactly 0 (R9).
+ *
+ * Mapping: LPA = 8 lanes per atom read the atom's CSR row in 32-byte pieces (coalesced sector
+ * reads), gather x~_j as one float4 / double4 from the pos4 array (L1/L2 resident per system),
+ * xor-shuffle over the 8 lanes, then a warp-level segmented reduction of E and W into the fp64
+ * per-system outputs (one atomic per warp when the warp sits inside one system).
+ */
+#include "ts_internal.cuh"
+
+#define LPA 8
+
+template <typename T> __device__ __forceinline__ T t_exp(T x);
+template <> __device__ __forceinline__ float t_exp<float>(float x) { return expf(x); }
+template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
+template <typename T> __device__ __forceinline__ T t_pow(T x, T a);
+template <> __device__ __forceinline__ float t_pow<float>(float x, float a) { return powf(x, a); }
+template <> __device__ __forceinline__ double t_pow<double>(double x, double a) { return pow(x, a); }
+template <typename T> __device__ __forceinline__ T t_sqrt(T x);
+template <> __device__ __forceinline__ float t_sqrt<float>(float x) { return sqrtf(x); }
+template <> __device__ __forceinline__ double t_sqrt<double>(double x) { return sqrt(x); }
+
+/* V (shifted) and g = V'(r)/r for r^2 < rc^2. */
+template <typename T, int KIND>
+__device__ __forceinline__ void pot_eval(const PotEntry<T> &pe, T r2, T &V, T &g)
+{
+    if (KIND == TS_LJ) {
+        T ir2 = (T)1 / r2;
+        T ir6 = ir2 * ir2 * ir2;
+        T a = pe.c0 * ir6 * ir6, b = pe.c1 * ir6;
+        V = (a - b) - pe.vshift;
+        g = -((T)12 * a - (T)6 * b) * ir2;
+    } else if (KIND == TS_MORSE) {
+        T r = t_sqrt<T>(r2);
+        T e = t_exp<T>(-pe.p1 * (r - pe.p2));
+        T om = (T)1 - e;
+        V = pe.p0 * (om * om - (T)1) - pe.vshift;
+        g = pe.c0 * om * e / r;
+    } else {
+        T r = t_sqrt<T>(r2);
+        T u = (T)1 - r * pe.c2;
+        if (u <= (T)0) { V = (T)0; g = (T)0; return; }
+        T um1;                       /* u^(alpha-1) */
+        T al = pe.p2;
+        if (al == (T)2) um1 = u;
+        else if (al == (T)1) um1 = (T)1;
+        else if (al == (T)3) um1 = u * u;
+        else um1 = t_pow<T>(u, al - (T)1);
+        V = pe.c0 * um1 * u - pe.vshift;
+        g = -pe.c1 * um1 / r;
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ int type_of(const typename Vec4<T>::type &q)
+{
+    if (sizeof(T) == 4) return __float_as_int((float)q.w);
+    return (int)__double_as_longlong((double)q.w);
+}
+
+template <typename T, int KIND, bool EV>
+__global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
+{
+    typedef typename Vec4<T>::type V4;
+    const unsigned FULL = 0xffffffffu;
+    long long gid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long i = gid / LPA;
+    int sub = threadIdx.x & (LPA - 1);
+    bool valid = i < d.N;
+    int s = valid ? d.sysidx[i] : -1;
+    bool act = valid && !(masked && !d.sys_active[s]) && d.nbr_len[s] >= 0;
+    const V4 *pos4 = (const V4 *)d.pos4;
+    const PotEntry<T> *tab = (const PotEntry<T> *)d.pot;
+    int nt = d.n_types;
+    T fx = 0, fy = 0, fz = 0, e = 0, w0 = 0, w1 = 0, w2 = 0, w3 = 0, w4 = 0, w5 = 0;
+    if (act) {
+        const T *h = (const T *)d.hT + 9 * (size_t)s;
+        T h0 = __ldg(h), h1 = __ldg(h + 1), h2 = __ldg(h + 2), h3 = __ldg(h + 3), h4 = __ldg(h + 4),
+          h5 = __ldg(h + 5), h6 = __ldg(h + 6), h7 = __ldg(h + 7), h8 = __ldg(h + 8);
+        V4 xi = pos4[i];
+        int ti = type_of<T>(xi);
+        int a0 = d.sysoff[s];
+        const unsigned *row = d.nbr + d.nbr_off[i];
+        int cnt = d.nbr_cnt[i];
+        PotEntry<T> pe = tab[ti * nt];
+#pragma unroll 2
+        for (int k = sub; k < cnt; k += LPA) {
+            unsigned en = __ldg(row + k);
+            int j = (int)(en & TS_J_MASK);
+            int s0, s1, s2;
+            ts_unpack_shift(en, s0, s1, s2);
+            V4 xj = pos4[a0 + j];
+            T f0 = (T)s0, f1 = (T)s1, f2 = (T)s2;
+            T rx = (xj.x - xi.x) + (f0 * h0 + f1 * h3 + f2 * h6);
+            T ry = (xj.y - xi.y) + (f0 * h1 + f1 * h4 + f2 * h7);
+            T rz = (xj.z - xi.z) + (f0 * h2 + f1 * h5 + f2 * h8);
+            T r2 = rx * rx + ry * ry + rz * rz;
+            if (nt > 1) pe = tab[ti * nt + type_of<T>(xj)];
+            if (r2 < pe.rc2) {
+                T V, g;
+                pot_eval<T, KIND>(pe, r2, V, g);
+                fx += g * rx; fy += g * ry; fz += g * rz;
+                if (EV) {
+                    e += V;
+                    T gx = g * rx, gy = g * ry;
+                    w0 += gx * rx; w1 += gx * ry; w2 += gx * rz;
+                    w3 += gy * ry; w4 += gy * rz; w5 += g * rz * rz;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 1; o < LPA; o <<= 1) {
+        fx += __shfl_xor_sync(FULL, fx, o);
+        fy += __shfl_xor_sync(FULL, fy, o);
+        fz += __shfl_xor_sync(FULL, fz, o);
+    }
+    if (act && sub == 0) {
+        T *f = (T *)d.force + 3 * i;
+        f[0] = fx; f[1] = fy; f[2] = fz;
+        if (!(fabs((double)fx) + fabs((double)fy) + fabs((double)fz) < 1e300))
+            atomicOr(&d.status->flags, TS_FLAG_NONFINITE);
+    }
+    if (EV) {
+        /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
+        double acc[7] = { 0.5 * (double)e, -0.5 * (double)w0, -0.5 * (double)w1, -0.5 * (double)w2,
+                          -0.5 * (double)w3, -0.5 * (double)w4, -0.5 * (double)w5 };
+        int key = act ? s : -1;
+        int sl = __shfl_sync(FULL, key, 0);
+        /* warp inside one system: full warp reduction, one set of atomics */
+        bool whole = __all_sync(FULL, key == sl) && sl >= 0;
+        if (whole) {
+#pragma unroll
+            for (int q = 0; q < 7; ++q)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
+            if ((threadIdx.x & 31) == 0) {
+                atomicAdd(&d.energy[sl], acc[0]);
+                if (d.virial) {
+                    double *W = d.virial + 9 * (size_t)sl;
+                    atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
+                    atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
+                    atomicAdd(&W[6], acc[3]); atomicAdd(&W[7], acc[5]); atomicAdd(&W[8], acc[6]);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 7; ++q)
+#pragma unroll
+                for (int o = 1; o < LPA; o <<= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
+            if (act && sub == 0) {
+                atomicAdd(&d.energy[s], acc[0]);
+                if (d.virial) {
+                    double *W = d.virial + 9 * (size_t)s;
+                    atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
+                    atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
+                    atomicAdd(&W[6], acc[3]); atomicAdd(&W[7], acc[5]); atomicAdd(&W[8], acc[6]);
+                }
+            }
+        }
+    }
+}
+
+/* zero E / W of the systems whose forces are about to be recomputed */
+__global__ void k_zero_ev(DevState d, int masked, unsigned want)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= d.S) return;
+    if (masked && !d.sys_active[s]) return;
+    if (d.nbr_len[s] < 0) return;
+    d.energy[s] = 0.0;
+    if ((want & TS_WANT_VIRIAL) && d.virial)
+        for (int k = 0; k < 9; ++k) d.virial[9 * (size_t)s + k] = 0.0;
+}
+
+template <typename T, int KIND>
+static void launch_pair_k(ts_state *st, unsigned want, bool masked, cudaStream_t q)
+{
+    DevState d = st->d;
+    long long nthreads = d.N * LPA;
+    unsigned nb = (unsigned)((nthreads + 255) / 256);
+    if (want) {
+        if (!(want & TS_WANT_VIRIAL)) d.virial = nullptr;
+        k_zero_ev<<<(d.S + 127) / 128, 128, 0, q>>>(d, masked ? 1 : 0, want);
+        k_pair<T, KIND, true><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        st->launches += 2;
+    } else {
+        k_pair<T, KIND, false><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        st->launches += 1;
+    }
+}
+
+void launch_pair(ts_state *st, unsigned want, bool masked, cudaStream_t q)
+{
+    int kind = st->d.kind;
+    if (st->d.dtype == TS_F32) {
+        if (kind == TS_LJ) launch_pair_k<float, TS_LJ>(st, want, masked, q);
+        else if (kind == TS_MORSE) launch_pair_k<float, TS_MORSE>(st, want, masked, q);
+        else launch_pair_k<float, TS_SOFT_SPHERE>(st, want, masked, q);
+    } else {
+        if (kind == TS_LJ) launch_pair_k<double, TS_LJ>(st, want, masked, q);
+        else if (kind == TS_MORSE) launch_pair_k<double, TS_MORSE>(st, want, masked, q);
+        else launch_pair_k<double, TS_SOFT_SPHERE>(st, want, masked, q);
+    }
+}

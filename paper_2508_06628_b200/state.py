@@ -1,0 +1,157 @@
+"""SimState: the caller-owned device arrays of one ragged batch plus its libts handle.
+
+PyTorch provides device memory and the stream; all computation happens behind the C ABI.
+"""
+import ctypes as C
+
+import numpy as np
+
+import paper_2508_06628_b200 as ts
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2508_06628_b200 needs a CUDA device (there is no CPU fallback)")
+    return torch
+
+
+class _Pot:
+    """Host tables of a potential, kept alive for ts_state_create."""
+
+    def __init__(self, pot):
+        self.kind = pot.kind if isinstance(pot.kind, int) else ts.KINDS[pot.kind]
+        self.n_types = int(pot.n_types)
+        nt2 = self.n_types ** 2
+        self.arrs = [np.ascontiguousarray(np.asarray(getattr(pot, k), dtype=np.float64).reshape(nt2))
+                     for k in ("p0", "p1", "p2", "rc")]
+        p = [a.ctypes.data_as(C.c_void_p) for a in self.arrs]
+        self.c = ts.ts_potential(self.kind, self.n_types, p[0], p[1], p[2], p[3], int(bool(pot.shift_energy)))
+
+
+class SimState:
+    """One batch on the device.  `batch` is duck-typed (workloads.Batch): pos, vel, mass, type,
+    system_idx, cell, potential, mass_conv, kB, skin, sys_uid."""
+
+    def __init__(self, batch, dtype=None, skin=None, slack=1.25, device="cuda:0", engine=None, pinned_src=None):
+        torch = _torch()
+        self.torch = torch
+        self.device = torch.device(device)
+        dtype = dtype or getattr(batch, "dtype", "f64")
+        self.dtype = ts.TS_F32 if dtype in ("f32", ts.TS_F32) else ts.TS_F64
+        self.tdtype = torch.float32 if self.dtype == ts.TS_F32 else torch.float64
+        self.npdtype = np.float32 if self.dtype == ts.TS_F32 else np.float64
+        self.N = int(np.asarray(batch.pos).shape[0])
+        self.S = int(np.asarray(batch.cell).shape[0])
+        self.skin = float(batch.skin if skin is None else skin)
+        self.slack = float(slack)
+        self.units = ts.ts_units(float(batch.mass_conv), float(batch.kB))
+        self._pot = _Pot(batch.potential)
+        dev = self.device
+
+        def up(a, dt, shape):
+            t = torch.from_numpy(np.ascontiguousarray(np.asarray(a).reshape(shape))).to(dt)
+            return t.to(dev, non_blocking=False).contiguous()
+
+        self.pos = up(batch.pos, self.tdtype, (self.N, 3))
+        vel = batch.vel if getattr(batch, "vel", None) is not None else np.zeros((self.N, 3))
+        self.vel = up(vel, self.tdtype, (self.N, 3))
+        self.mass = up(batch.mass, self.tdtype, (self.N,))
+        self.type = up(batch.type, torch.int32, (self.N,))
+        self.system_idx = up(batch.system_idx, torch.int32, (self.N,))
+        self.cell = up(batch.cell, self.tdtype, (self.S, 3, 3))
+        self.force = torch.zeros((self.N, 3), dtype=self.tdtype, device=dev)
+        self.energy = torch.zeros(self.S, dtype=torch.float64, device=dev)
+        self.virial = torch.zeros((self.S, 3, 3), dtype=torch.float64, device=dev)
+        self.kinetic = torch.zeros(self.S, dtype=torch.float64, device=dev)
+        uid = getattr(batch, "sys_uid", None)
+        self.sys_uid = None if uid is None else torch.from_numpy(np.asarray(uid).astype(np.int64)).to(torch.int32).to(dev)
+        self.desc = self._make_desc()
+        self.nbr = ts.ts_nbr_params(self.skin, self.slack)
+        with torch.cuda.device(self.device):
+            self.workspace_bytes = ts.ts_workspace_bytes(self.desc, self._pot.c, self.nbr)
+            self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=dev)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            self.handle = ts.ts_state_create(self.desc, self._pot.c, self.nbr, self._ws_ptr, self.workspace_bytes)
+        if engine is not None:
+            ts.ts_set_engine(self.handle, int(engine))
+
+    def _make_desc(self):
+        p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        return ts.ts_state_desc(self.N, self.S, self.dtype, self.units, p(self.pos), p(self.vel), p(self.force),
+                                p(self.mass), p(self.type), p(self.system_idx), p(self.cell), p(self.energy),
+                                p(self.virial), p(self.kinetic), p(self.sys_uid))
+
+    def close(self):
+        if getattr(self, "handle", None) is not None:
+            self.torch.cuda.synchronize(self.device)
+            ts.ts_state_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ C-ABI calls
+    def build_neighbors(self):
+        ts.ts_build_neighbors(self.handle)
+
+    def compute_forces(self, want=ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL):
+        ts.ts_compute_forces(self.handle, want)
+
+    def md_step(self, params, n_steps, want=ts.TS_WANT_ENERGY):
+        if isinstance(params, dict):
+            params = ts.md_params(**params)
+        ts.ts_md_step(self.handle, params, n_steps, want)
+
+    def fire_step(self, params, n_steps):
+        if isinstance(params, dict):
+            params = ts.fire_params(**params)
+        ts.ts_fire_step(self.handle, params, n_steps)
+
+    def poll(self):
+        return ts.ts_poll(self.handle)
+
+    def converged_mask(self):
+        return ts.ts_converged_mask(self.handle, self.S)
+
+    def get_neighbors(self):
+        return ts.ts_get_neighbors(self.handle, self.N)
+
+    def set_system_steps(self, steps):
+        ts.ts_set_system_steps(self.handle, steps)
+
+    def get_system_steps(self):
+        return ts.ts_get_system_steps(self.handle, self.S)
+
+    def set_engine(self, engine):
+        ts.ts_set_engine(self.handle, engine)
+
+    def launch_count(self):
+        return ts.ts_launch_count(self.handle)
+
+    def swap_systems(self, slots, fresh):
+        """Replace the systems in `slots` by those of `fresh` (duck-typed batch, same sizes)."""
+        torch = self.torch
+        n = len(slots)
+        nat = int(np.asarray(fresh.pos).shape[0])
+        dev = self.device
+
+        def up(a, dt, shape):
+            return torch.from_numpy(np.ascontiguousarray(np.asarray(a).reshape(shape))).to(dt).to(dev).contiguous()
+
+        keep = [up(fresh.pos, self.tdtype, (nat, 3)), up(fresh.vel, self.tdtype, (nat, 3)),
+                up(fresh.mass, self.tdtype, (nat,)), up(fresh.type, torch.int32, (nat,)),
+                up(fresh.cell, self.tdtype, (n, 3, 3)),
+                torch.from_numpy(np.asarray(fresh.sys_uid).astype(np.int64)).to(torch.int32).to(dev)]
+        p = lambda t: C.c_void_p(t.data_ptr())
+        d = ts.ts_state_desc(nat, n, self.dtype, self.units, p(keep[0]), p(keep[1]), None, p(keep[2]), p(keep[3]),
+                             None, p(keep[4]), None, None, None, p(keep[5]))
+        ts.ts_swap_systems(self.handle, slots, d)   # synchronises: `keep` may be released afterwards
+
+    # ------------------------------------------------------------------ host views
+    def numpy(self, name):
+        return getattr(self, name).detach().cpu().numpy()

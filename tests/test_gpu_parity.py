@@ -1,0 +1,184 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are BASELINE.json:north_star's: pair sets bit-exact; fp64 E rel
+1e-12, F abs 1e-10, x after 100 steps 1e-8; fp32 F within 1e-4 of the system's max |F|, E rel 1e-5
+(R31: relative to max(|E|, sum 1/2 |V|))."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ts():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2508_06628_b200 as m
+    m.lib()
+    return m
+
+
+ENGINES = [0, 1]
+
+
+def _cases():
+    """Small batches shaped like the five configs: several tiles, ragged tails, tiny sheared boxes."""
+    c = {}
+    c["cfg1_f64"] = lambda: wl.cfg1(n_systems=4)
+    c["cfg2_f32"] = lambda: wl.cfg2(n_systems=3, dtype="f32")
+    c["cfg2_f64"] = lambda: wl.cfg2(n_systems=2, dtype="f64")
+    c["cfg3_f32"] = lambda: wl.cfg3(n_systems=12, dtype="f32", n_range=(32, 700))
+    c["cfg3_f64"] = lambda: wl.cfg3(n_systems=8, dtype="f64", n_range=(32, 400))
+    c["cfg4_f64"] = lambda: wl.cfg4(range(6))
+    c["tiny_f64"] = lambda: wl.cfg1(n_systems=2, reps=1)       # 4 atoms, box 5.26 A << r_c: self images
+    c["small_f64"] = lambda: wl.cfg1(n_systems=3, reps=2)      # 32 atoms, box 10.52 A < 2 r_list
+    return c
+
+
+CASES = _cases()
+
+
+def _pair_sets(orc, b, R):
+    out = []
+    for s in range(b.n_systems):
+        a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+        i, j, S, _ = orc.pairs(b.pos[a0:a1], b.cell[s], R)
+        out.append(set(zip((i + a0).tolist(), (j + a0).tolist(), S[:, 0].tolist(), S[:, 1].tolist(), S[:, 2].tolist())))
+    return out
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_neighbour_pair_sets_bit_exact(ts, orc, name):
+    b = CASES[name]()
+    st = ts.SimState(b, engine=0)
+    st.build_neighbors()
+    off, j, shift = st.get_neighbors()
+    rep = st.poll()
+    assert rep.flags == 0 and rep.list_valid == 1
+    i = np.repeat(np.arange(b.n_atoms), np.diff(off))
+    got = set(zip(i.tolist(), j.tolist(), shift[:, 0].tolist(), shift[:, 1].tolist(), shift[:, 2].tolist()))
+    assert len(got) == j.size                                  # no duplicate (i, j, S)
+    want = set().union(*_pair_sets(orc, b, b.r_list))
+    assert got == want
+    assert rep.nnz == len(want) and rep.nnz <= rep.nnz_capacity
+    assert rep.max_neighbors == int(np.diff(off).max())
+    st.close()
+
+
+def _check_efw(b, st, o, fp32):
+    E, F, W = st.numpy("energy"), st.numpy("force").astype(np.float64), st.numpy("virial")
+    scale = np.maximum(np.abs(o["E"]), o["Eabs"])
+    if fp32:
+        assert np.all(np.abs(E - o["E"]) <= 1e-5 * scale)
+        for s in range(b.n_systems):
+            a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+            fmax = np.linalg.norm(o["F"][a0:a1], axis=1).max()
+            assert np.abs(F[a0:a1] - o["F"][a0:a1]).max() <= 1e-4 * fmax
+        wscale = np.abs(o["W"]).reshape(b.n_systems, -1).max(1) + o["Eabs"]
+        assert np.all(np.abs(W - o["W"]).reshape(b.n_systems, -1).max(1) <= 1e-4 * wscale)
+    else:
+        assert np.all(np.abs(E - o["E"]) <= 1e-12 * scale)
+        assert np.abs(F - o["F"]).max() <= 1e-10
+        wscale = np.abs(o["W"]).reshape(b.n_systems, -1).max(1) + o["Eabs"]
+        assert np.all(np.abs(W - o["W"]).reshape(b.n_systems, -1).max(1) <= 1e-11 * wscale)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_energy_forces_virial(ts, orc, name):
+    b = CASES[name]()
+    o = orc.energy_forces(b)
+    st = ts.SimState(b, engine=0)
+    st.compute_forces(ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    assert st.poll().flags == 0
+    _check_efw(b, st, o, b.dtype == "f32")
+    KE = st.numpy("kinetic")
+    assert np.allclose(KE, orc.kinetic(b), rtol=1e-6 if b.dtype == "f32" else 1e-13, atol=1e-300)
+    st.close()
+
+
+def test_results_do_not_depend_on_skin(ts, orc):
+    b = CASES["cfg1_f64"]()
+    o = orc.energy_forces(b)
+    for skin in (0.0, 0.3, 1.2):
+        st = ts.SimState(b, skin=skin, engine=0)
+        st.compute_forces()
+        _check_efw(b, st, o, False)
+        st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_nve_100_steps_fp64_cfg1(ts, orc, engine):
+    b = wl.cfg1(n_systems=4)
+    o = orc.md_run(b, "nve", 2.0, 100)
+    st = ts.SimState(b, engine=engine)
+    st.md_step(b.md, 100)
+    rep = st.poll()
+    assert rep.flags == 0
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
+    assert np.abs(st.numpy("force") - o["F"]).max() <= 1e-9
+    assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-10)
+    assert np.allclose(st.numpy("kinetic"), o["KE"], rtol=1e-10)
+    assert np.array_equal(st.get_system_steps(), np.full(4, 100, np.uint64))
+    st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_baoab_100_steps_fp64_cfg2(ts, orc, engine):
+    b = wl.cfg2(n_systems=2, dtype="f64")
+    md = dict(b.md)
+    o = orc.md_run(b, "baoab", md["dt"], 100, temperature=md["temperature"], friction=md["friction"],
+                   seed=md["seed"], sys_uid=b.sys_uid)
+    st = ts.SimState(b, engine=engine)
+    st.md_step(md, 60)
+    st.md_step(md, 40)                                         # split call: per-system step counter carries on (R18)
+    assert st.poll().flags == 0
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
+    assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-9)
+    st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_nve_morse_triclinic_fp64(ts, orc, engine):
+    b = wl.cfg3(n_systems=6, dtype="f64", n_range=(32, 300))
+    o = orc.md_run(b, "nve", 1.0, 100)
+    st = ts.SimState(b, engine=engine)
+    st.md_step(dict(b.md), 100, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.n_rebuilds >= 1
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-9)
+    assert np.abs(st.numpy("virial") - o["W"]).max() <= 1e-8 * np.abs(o["W"]).max()
+    st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_fp32_replay_parity_after_md(ts, orc, engine):
+    """R29: after k fp32 steps the GPU's own positions are fed to the oracle; forces must agree to
+    1e-4 of max|F| except for atoms in a pair within 1e-5 A of r_c (counted, not compared)."""
+    b = wl.cfg2(n_systems=2, dtype="f32")
+    st = ts.SimState(b, engine=engine)
+    st.md_step(dict(b.md), 50)
+    assert st.poll().flags == 0
+    bb = wl.with_(b, pos=st.numpy("pos").astype(np.float64), vel=st.numpy("vel").astype(np.float64))
+    o = orc.energy_forces(bb)
+    F = st.numpy("force").astype(np.float64)
+    rc = b.potential.rc_max
+    dont_care = np.zeros(b.n_atoms, bool)
+    for s in range(b.n_systems):
+        a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+        i, j, S, r2 = orc.pairs(bb.pos[a0:a1], bb.cell[s], rc + 1e-3)
+        near = np.abs(np.sqrt(r2) - rc) < 1e-5
+        dont_care[a0 + i[near]] = True
+    assert dont_care.mean() < 0.01
+    for s in range(b.n_systems):
+        a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+        ok = ~dont_care[a0:a1]
+        fmax = np.linalg.norm(o["F"][a0:a1], axis=1).max()
+        assert np.abs(F[a0:a1] - o["F"][a0:a1])[ok].max() <= 1e-4 * fmax
+    scale = np.maximum(np.abs(o["E"]), o["Eabs"])
+    assert np.all(np.abs(st.numpy("energy") - o["E"]) <= 2e-5 * scale)
+    st.close()
