@@ -121,13 +121,16 @@ typedef struct {
 typedef struct {
     uint32_t flags;          /* TS_FLAG_* sticky bits */
     int32_t n_rebuilds;      /* neighbour builds since create */
-    int64_t nnz;             /* directed pairs in the current list */
+    int64_t nnz;             /* directed pairs in the current list (resident engine: summed over the systems' lists) */
     int64_t nnz_capacity;
     int64_t steps_done;      /* MD/FIRE steps enqueued since create */
     int32_t n_converged;     /* systems with FIRE status converged */
     int32_t n_failed;        /* systems that hit max_steps */
-    int32_t max_neighbors;   /* longest row of the current list */
+    int32_t max_neighbors;   /* longest row of the current list (general engine) */
     int32_t list_valid;
+    int64_t resident_rebuilds; /* resident engine: per-system list builds since create, summed over systems */
+    int32_t engine;          /* engine that ran the last stepping call: 0 general, 1 resident */
+    int32_t reserved;
 } ts_report;
 
 /* Bytes of workspace ts_state_create needs for this batch (the memory-estimate primitive, SURVEY

@@ -66,7 +66,8 @@ class ts_fire_params(C.Structure):
 class ts_report(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("n_rebuilds", C.c_int32), ("nnz", C.c_int64), ("nnz_capacity", C.c_int64),
                 ("steps_done", C.c_int64), ("n_converged", C.c_int32), ("n_failed", C.c_int32),
-                ("max_neighbors", C.c_int32), ("list_valid", C.c_int32)]
+                ("max_neighbors", C.c_int32), ("list_valid", C.c_int32), ("resident_rebuilds", C.c_int64),
+                ("engine", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None

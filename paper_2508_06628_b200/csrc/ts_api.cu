@@ -272,6 +272,7 @@ extern "C" ts_status ts_state_create(const ts_state_desc *desc, const ts_potenti
 extern "C" ts_status ts_state_destroy(ts_state *st)
 {
     if (!st) return TS_ERR_INVALID_ARG;
+    resident_free(st);
     free(st->h_sysoff);
     free(st);
     return TS_OK;

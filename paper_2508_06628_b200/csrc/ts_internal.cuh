@@ -51,6 +51,8 @@ struct DevStatus {
     unsigned long long nnz;
     unsigned int list_valid;
     unsigned int pad;
+    unsigned long long res_nnz;       /* resident engine: pairs in the lists at the end of the last call */
+    unsigned long long res_rebuilds;  /* resident engine: per-system list builds, summed over systems    */
 };
 
 /* Everything a kernel needs, passed by value (well under the 4 KB parameter limit). */
@@ -105,6 +107,8 @@ struct ts_state {
     bool list_built;             /* a build has been enqueued and no swap since */
     bool forces_current;
     int engine;
+    int last_engine;             /* engine that ran the last stepping call */
+    void *res_plan;              /* resident engine launch plan (ts_resident.cu) */
     long long launches;
     long long steps_done;
     unsigned int seen_flags;     /* last flags seen by ts_poll         */
@@ -149,7 +153,9 @@ void launch_fire_post(ts_state *st, const ts_fire_params &p, cudaStream_t q);
 void launch_fire_count(ts_state *st, cudaStream_t q);
 void launch_swap(ts_state *st, int n, const ts_state_desc *fresh, cudaStream_t q);
 /* ts_resident.cu */
-bool resident_supported(const ts_state *st);
+bool resident_supported(ts_state *st);
+void resident_invalidate(ts_state *st);
+void resident_free(ts_state *st);
 ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q);
 
 /* ------------------------------------------------------------------ device helpers */

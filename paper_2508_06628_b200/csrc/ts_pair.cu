@@ -11,49 +11,9 @@
  * per-system outputs (one atomic per warp when the warp sits inside one system).
  */
 #include "ts_internal.cuh"
+#include "ts_pot.cuh"
 
 #define LPA 8
-
-template <typename T> __device__ __forceinline__ T t_exp(T x);
-template <> __device__ __forceinline__ float t_exp<float>(float x) { return expf(x); }
-template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
-template <typename T> __device__ __forceinline__ T t_pow(T x, T a);
-template <> __device__ __forceinline__ float t_pow<float>(float x, float a) { return powf(x, a); }
-template <> __device__ __forceinline__ double t_pow<double>(double x, double a) { return pow(x, a); }
-template <typename T> __device__ __forceinline__ T t_sqrt(T x);
-template <> __device__ __forceinline__ float t_sqrt<float>(float x) { return sqrtf(x); }
-template <> __device__ __forceinline__ double t_sqrt<double>(double x) { return sqrt(x); }
-
-/* V (shifted) and g = V'(r)/r for r^2 < rc^2. */
-template <typename T, int KIND>
-__device__ __forceinline__ void pot_eval(const PotEntry<T> &pe, T r2, T &V, T &g)
-{
-    if (KIND == TS_LJ) {
-        T ir2 = (T)1 / r2;
-        T ir6 = ir2 * ir2 * ir2;
-        T a = pe.c0 * ir6 * ir6, b = pe.c1 * ir6;
-        V = (a - b) - pe.vshift;
-        g = -((T)12 * a - (T)6 * b) * ir2;
-    } else if (KIND == TS_MORSE) {
-        T r = t_sqrt<T>(r2);
-        T e = t_exp<T>(-pe.p1 * (r - pe.p2));
-        T om = (T)1 - e;
-        V = pe.p0 * (om * om - (T)1) - pe.vshift;
-        g = pe.c0 * om * e / r;
-    } else {
-        T r = t_sqrt<T>(r2);
-        T u = (T)1 - r * pe.c2;
-        if (u <= (T)0) { V = (T)0; g = (T)0; return; }
-        T um1;                       /* u^(alpha-1) */
-        T al = pe.p2;
-        if (al == (T)2) um1 = u;
-        else if (al == (T)1) um1 = (T)1;
-        else if (al == (T)3) um1 = u * u;
-        else um1 = t_pow<T>(u, al - (T)1);
-        V = pe.c0 * um1 * u - pe.vshift;
-        g = -pe.c1 * um1 / r;
-    }
-}
 
 template <typename T>
 __device__ __forceinline__ int type_of(const typename Vec4<T>::type &q)
@@ -100,16 +60,20 @@ __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
             T rz = (xj.z - xi.z) + (f0 * h2 + f1 * h5 + f2 * h8);
             T r2 = rx * rx + ry * ry + rz * rz;
             if (nt > 1) pe = tab[ti * nt + type_of<T>(xj)];
-            if (r2 < pe.rc2) {
+            const bool in = r2 < pe.rc2;     /* pairs in the Verlet shell contribute exactly 0 (R9) */
+            if (EV) {
                 T V, g;
                 pot_eval<T, KIND>(pe, r2, V, g);
+                g = in ? g : (T)0; V = in ? V : (T)0;
                 fx += g * rx; fy += g * ry; fz += g * rz;
-                if (EV) {
-                    e += V;
-                    T gx = g * rx, gy = g * ry;
-                    w0 += gx * rx; w1 += gx * ry; w2 += gx * rz;
-                    w3 += gy * ry; w4 += gy * rz; w5 += g * rz * rz;
-                }
+                e += V;
+                T gx = g * rx, gy = g * ry;
+                w0 += gx * rx; w1 += gx * ry; w2 += gx * rz;
+                w3 += gy * ry; w4 += gy * rz; w5 += g * rz * rz;
+            } else {
+                T g = pot_force<T, KIND>(pe, r2);
+                g = in ? g : (T)0;
+                fx += g * rx; fy += g * ry; fz += g * rz;
             }
         }
     }

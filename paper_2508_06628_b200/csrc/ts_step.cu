@@ -50,6 +50,7 @@ extern "C" ts_status ts_compute_forces(ts_state *st, uint32_t want, void *stream
 {
     NEED_STATE(st);
     cudaStream_t q = (cudaStream_t)stream;
+    st->last_engine = 0;
     ensure_list(st, q);
     launch_pair(st, want & 3u, false, q);
     if (want & TS_WANT_ENERGY) launch_kinetic(st, q);
@@ -79,6 +80,7 @@ extern "C" ts_status ts_md_step(ts_state *st, const ts_md_params *p, int32_t n_s
             return rc;
         }
     }
+    st->last_engine = 0;
     if (!st->forces_current || n_steps == 0) {
         ensure_list(st, q);
         launch_pair(st, n_steps == 0 ? want : 0u, false, q);
@@ -101,6 +103,7 @@ extern "C" ts_status ts_fire_step(ts_state *st, const ts_fire_params *p, int32_t
     NEED_STATE(st);
     if (!p || n_steps < 0 || !(p->dt_start > 0.0) || !(p->dt_max > 0.0) || !(p->f_max > 0.0)) return TS_ERR_INVALID_ARG;
     cudaStream_t q = (cudaStream_t)stream;
+    st->last_engine = 0;
     launch_fire_init(st, *p, q);
     ensure_list(st, q);
     launch_pair(st, TS_WANT_ENERGY, true, q);
@@ -129,7 +132,9 @@ extern "C" ts_status ts_poll(ts_state *st, ts_report *out, void *stream)
     memset(out, 0, sizeof *out);
     out->flags = hs.flags;
     out->n_rebuilds = (int32_t)hs.n_rebuilds;
-    out->nnz = (int64_t)hs.nnz;
+    out->nnz = st->last_engine == 1 ? (int64_t)hs.res_nnz : (int64_t)hs.nnz;
+    out->resident_rebuilds = (int64_t)hs.res_rebuilds;
+    out->engine = st->last_engine;
     out->nnz_capacity = st->d.nbr_cap;
     out->steps_done = st->steps_done;
     out->n_converged = cnt[0];
@@ -191,7 +196,7 @@ extern "C" ts_status ts_swap_systems(ts_state *st, const int32_t *slots, int32_t
     if (off != fresh->n_atoms) return TS_ERR_INVALID_ARG;
     TS_CUDA_OK(st, cudaMemcpyAsync(st->d.scratch, up.data(), sizeof(int) * up.size(), cudaMemcpyHostToDevice, q));
     launch_swap(st, n, fresh, q);
-    if (fresh->cell) launch_geometry(st, 0, n, st->d.scratch, q);
+    if (fresh->cell) { launch_geometry(st, 0, n, st->d.scratch, q); resident_invalidate(st); }
     st->list_built = false;
     st->forces_current = false;
     /* the upload buffer must outlive the copy */
