@@ -27,6 +27,9 @@ sys.path.insert(0, ROOT)
 
 import workloads as wl  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per k_resident_md launch (100 MD steps), profiles/r01_ncu_resident_cfg2_fp32.md
+NCU_TRAFFIC = {"resident": 1.888256e6 + 256.0, "general": None}
+
 METRIC = "atom_steps_per_s"
 UNIT = "atom-steps/s"
 
@@ -82,9 +85,24 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def rank_system_ids(rank, n_systems):
+    """Weak scaling: rank r steps its own systems r*n .. (r+1)*n - 1 (independent units, no exchange step)."""
+    return list(range(rank * n_systems, (rank + 1) * n_systems))
+
+
 def make_batch(rank, n_systems):
-    ids = list(range(rank * n_systems, (rank + 1) * n_systems))
-    return wl.cfg2(n_systems=n_systems, dtype="f32", system_ids=ids)
+    return wl.cfg2(n_systems=n_systems, dtype="f32", system_ids=rank_system_ids(rank, n_systems))
+
+
+def max_over_ranks(times, world, device):
+    """Device times -> max over ranks (the only collective of the job; NCCL on GPUs, gloo in the CPU test)."""
+    if world == 1:
+        return [float(t) for t in times]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
 
 
 def algorithmic_model(nbar, K, w=4, entry_bytes=4):
@@ -103,8 +121,8 @@ def run_reference(args):
         return
     import oracle
     cores = oracle.default_threads()
-    n_sys = min(64, cores)
-    md_steps = 2
+    n_sys = 64
+    md_steps = 10
     b = wl.cfg2(n_systems=n_sys, dtype="f32", clean=False)
     md = b.md
 
@@ -132,8 +150,8 @@ def run_reference(args):
 def cpu_baseline():
     import oracle
     cores = oracle.default_threads()
-    n_sys = min(64, cores)
-    md_steps = 8
+    n_sys = 64
+    md_steps = 150                                             # about 10-30 s of host work
     b = wl.cfg2(n_systems=n_sys, dtype="f32", clean=False)
     md = b.md
     t0 = time.perf_counter()
@@ -218,7 +236,7 @@ def main():
     e_a.record(stream)
     for _ in range(args.steps):
         st.pos.copy_(hpos, non_blocking=True); st.vel.copy_(hvel, non_blocking=True)
-        st.compute_forces(0)                                   # positions came from the host: forces are stale
+        st.invalidate()                                        # positions came from the host: forces are stale
         st.md_step(md, n_inner)
         hpos.copy_(st.pos, non_blocking=True); hvel.copy_(st.vel, non_blocking=True); hE.copy_(st.energy, non_blocking=True)
         stream.synchronize()
@@ -228,10 +246,7 @@ def main():
     h2d = 2 * st.pos.numel() * st.pos.element_size()
     d2h = h2d + st.energy.numel() * 8
 
-    if world > 1:
-        t = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_dev, t_e2e = float(t[0]), float(t[1])
+    t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], world, dev)
     atom_steps = float(st.N) * n_inner * args.steps * world
     value = atom_steps / t_dev
     steps_timed = n_inner * args.steps
@@ -259,7 +274,9 @@ def main():
         "e2e": {"value": atom_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src,
+                     "traffic": NCU_TRAFFIC.get("resident" if rep1.engine == 1 else "general"), "peak_source": peak_src,
+                     "traffic_note": "dram__bytes_read+write per launch from profiles/ (ncu --set full of this command); the resident "
+                                     "engine keeps systems on chip, so DRAM traffic is far below the algorithmic byte model",
                      "model": f"B_alg = {b_alg:.1f} B/atom-step (state 68 + {entry_bytes} B x nbar {nbar:.1f} + rebuild/K, K = {K:.1f}) "
                               f"x {st.N} atoms x {n_inner} MD steps per launch sequence",
                      "alu": {"flop_per_atom_step": flops, "achieved_tflops": flops * st.N * n_inner / (float(ms.mean()) * 1e-3) / 1e12,

@@ -199,8 +199,31 @@ ts_status ts_get_system_steps(ts_state *st, uint64_t *steps, void *stream);
  * to 0 otherwise.  Default 1.  Results obey the same tolerances either way.                       */
 ts_status ts_set_engine(ts_state *st, int32_t engine);
 
+/* Tell the library that the caller wrote desc.pos / desc.vel from outside (e.g. a host -> device
+ * copy): forces are stale and the list must be skin-checked against the new positions before the
+ * next step.  Host-side flag only, enqueues nothing.                                              */
+ts_status ts_invalidate(ts_state *st);
+
 /* Number of kernel launches enqueued by this state since create (for bench accounting).           */
 int64_t ts_launch_count(const ts_state *st);
+
+/* ---- host-side scheduling primitives (no device needed; all arrays HOST) ------------------------
+ * cost / scaler values are in any one unit (bytes from ts_estimate_system_bytes, or the paper's
+ * n_atoms / n_atoms_x_density memory scaler).                                        */
+
+/* In-flight admission: the longest prefix of cost[0..n) whose sum stays <= budget.  */
+ts_status ts_sched_fill(const double *cost, int64_t n, double budget, int64_t *n_taken, double *used);
+
+/* Figure 2 step 4: min over probes of n_systems[k] * scaler[k].                  */
+ts_status ts_sched_max_scaler(const int64_t *n_systems, const double *scaler, int32_t n_probes, double *out);
+
+/* BinningAutobatcher: first-fit-decreasing 1-D bin packing; bin_of[k] = bin of system
+ * k, *n_bins = bins used.  TS_ERR_INVALID_ARG if a system exceeds the capacity.                   */
+ts_status ts_sched_binpack(const double *cost, int64_t n, double capacity, int32_t *bin_of, int32_t *n_bins);
+
+/* Multi-GPU sharding by system (no exchange step): longest-processing-time-first
+ * assignment; rank_of[k] = rank of system k, load[r] = summed cost of rank r (may be NULL).        */
+ts_status ts_sched_partition(const double *cost, int64_t n, int32_t n_ranks, int32_t *rank_of, double *load);
 
 ts_status ts_clear_error(ts_state *st, void *stream);
 const char *ts_status_string(ts_status s);

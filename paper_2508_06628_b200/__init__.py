@@ -28,8 +28,9 @@ KINDS = {"lj": TS_LJ, "morse": TS_MORSE, "soft_sphere": TS_SOFT_SPHERE}
 EXPORTS = ["ts_workspace_bytes", "ts_estimate_system_bytes", "ts_state_create", "ts_state_destroy",
            "ts_build_neighbors", "ts_compute_forces", "ts_md_step", "ts_fire_step", "ts_poll",
            "ts_converged_mask", "ts_swap_systems", "ts_get_neighbors", "ts_set_system_steps",
-           "ts_get_system_steps", "ts_set_engine", "ts_launch_count", "ts_clear_error",
-           "ts_status_string", "ts_last_error"]
+           "ts_get_system_steps", "ts_set_engine", "ts_invalidate", "ts_launch_count", "ts_clear_error",
+           "ts_status_string", "ts_last_error", "ts_sched_fill", "ts_sched_max_scaler",
+           "ts_sched_binpack", "ts_sched_partition"]
 
 
 class ts_units(C.Structure):
@@ -205,8 +206,51 @@ def ts_set_engine(h, engine):
     _check(lib().ts_set_engine(h, C.c_int32(engine)), "ts_set_engine", h)
 
 
+def ts_invalidate(h):
+    _check(lib().ts_invalidate(h), "ts_invalidate", h)
+
+
 def ts_launch_count(h):
     return int(lib().ts_launch_count(h))
+
+
+# ------------------------------------------------------------------------------- host scheduling
+def _dptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def ts_sched_fill(cost, budget):
+    cost = np.ascontiguousarray(np.asarray(cost, dtype=np.float64))
+    n, used = C.c_int64(), C.c_double()
+    _check(lib().ts_sched_fill(_dptr(cost), C.c_int64(cost.size), C.c_double(budget), C.byref(n), C.byref(used)),
+           "ts_sched_fill")
+    return n.value, used.value
+
+
+def ts_sched_max_scaler(n_systems, scaler):
+    ns = np.ascontiguousarray(np.asarray(n_systems, dtype=np.int64))
+    sc = np.ascontiguousarray(np.asarray(scaler, dtype=np.float64))
+    out = C.c_double()
+    _check(lib().ts_sched_max_scaler(_dptr(ns), _dptr(sc), C.c_int32(ns.size), C.byref(out)), "ts_sched_max_scaler")
+    return out.value
+
+
+def ts_sched_binpack(cost, capacity):
+    cost = np.ascontiguousarray(np.asarray(cost, dtype=np.float64))
+    bins = np.zeros(cost.size, np.int32)
+    nb = C.c_int32()
+    _check(lib().ts_sched_binpack(_dptr(cost), C.c_int64(cost.size), C.c_double(capacity), _dptr(bins), C.byref(nb)),
+           "ts_sched_binpack")
+    return bins, nb.value
+
+
+def ts_sched_partition(cost, n_ranks):
+    cost = np.ascontiguousarray(np.asarray(cost, dtype=np.float64))
+    rank = np.zeros(cost.size, np.int32)
+    load = np.zeros(n_ranks, np.float64)
+    _check(lib().ts_sched_partition(_dptr(cost), C.c_int64(cost.size), C.c_int32(n_ranks), _dptr(rank), _dptr(load)),
+           "ts_sched_partition")
+    return rank, load
 
 
 def md_params(integrator="nve", dt=1.0, temperature=0.0, friction=0.0, seed=0, **_):

@@ -280,6 +280,13 @@ extern "C" ts_status ts_set_engine(ts_state *st, int32_t engine)
     return TS_OK;
 }
 
+extern "C" ts_status ts_invalidate(ts_state *st)
+{
+    if (!st) return TS_ERR_INVALID_ARG;
+    st->forces_current = false;
+    return TS_OK;
+}
+
 extern "C" int64_t ts_launch_count(const ts_state *st) { return st ? st->launches : 0; }
 
 extern "C" const char *ts_status_string(ts_status s)

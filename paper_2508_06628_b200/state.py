@@ -130,6 +130,9 @@ class SimState:
     def set_engine(self, engine):
         ts.ts_set_engine(self.handle, engine)
 
+    def invalidate(self):
+        ts.ts_invalidate(self.handle)
+
     def launch_count(self):
         return ts.ts_launch_count(self.handle)
 
