@@ -5,23 +5,30 @@
  * launch latency and on-chip bandwidth, not by HBM.  This engine therefore keeps a whole system on
  * chip for all n_steps of a ts_md_step call: one thread-block cluster of CL CTAs per system, each
  * CTA owning a contiguous slice of the system's atoms.  Per CTA, in shared memory:
- *     pos[2][N_s+1]  wrapped positions + type of ALL atoms of the system (double buffered; every
- *                    owner publishes its atom into every CTA of the cluster through DSMEM)
+ *     pos[NS]        wrapped positions + type of ALL atoms of the system (slots 0..N_s-1), eight
+ *                    far-away dummies (list padding, one per 16-byte bank group) and the GHOST
+ *                    slots: every periodic image of an atom that can lie within r_list of the cell
+ *                    (the atom is within r_list of a face) owns a slot holding x + S.h.  Every owner
+ *                    publishes its atom and its ghosts into every CTA of the cluster through DSMEM.
  *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only)
- *     rows[A][pitch] the Verlet list of the CTA's own atoms, 16-bit entries
+ *     gtab[N_s]      first ghost slot, active axes and image signs of every atom (rebuilds only)
+ *     rows[A][pitch] the Verlet list of the CTA's own atoms: 16-bit entries = byte offset of the
+ *                    neighbour's slot.  Thanks to the ghosts EVERY pair is a plain difference of two
+ *                    slots: no image arithmetic in the pair loop.
  *     fs[3][A]       forces of the own atoms (pair phase -> integrator phase)
- * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift.
- * HBM is touched when a system is loaded, when it is stored, and never in between.
+ * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift, ghost
+ * descriptor.  HBM is touched when a system is loaded, when it is stored, and never in between.
  *
- * One MD step = [owner: B A (O A) + publish + skin test] -> cluster barrier -> [rebuild if any
- * atom moved > skin/2] -> [pair phase] -> block barrier -> [owner: B].  Same physics as the
- * general engine.
+ * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading) -> [publish] -> cluster
+ * barrier -> [rebuild if any atom moved > skin/2] -> [pair phase] -> arrive(done reading) -> block
+ * barrier -> [owner: B].  Same physics as the general engine.
  *
- * Pair phase: 8 lanes per atom (one quarter-warp = one LDS.128 phase).  The list of an atom is
- * ordered at build time so that the 8 entries a quarter-warp fetches together point at 8 different
- * 16-byte bank groups (round-robin over j mod 8): the position gather is then conflict-free.  Home
- * pairs (image shift 0) and shifted pairs are kept in two segments so the home loop carries no
- * shift arithmetic; a home entry is the byte offset 16 j, a shifted entry is j | code << 11.
+ * Pair phase: 8 lanes per atom (one quarter-warp = one LDS.128 phase), two pairs per lane and
+ * iteration.  A ghost slot is congruent to its atom modulo 8 and lane l of the builder tests the
+ * candidates j = l mod 8, so a lane's hits all live in 16-byte bank group l; the list is laid out
+ * round-robin over the groups and the position gather is conflict-free while every group still has
+ * members.  The fp32 Lennard-Jones force-only loop uses Blackwell's packed FFMA2/FMUL2 (f32x2) on
+ * the two pairs of a lane: the kernel is issue-bound, and a packed op costs one issue slot.
  *
  * Rebuild: brute force over the system in fractional fixed point (integer subtraction wraps = the
  * minimum image), valid because the engine is only used when every cell height is >= 2 r_list
@@ -42,18 +49,18 @@ namespace cg = cooperative_groups;
 
 #define RES_MAX_THREADS 896         /* fp32; the fp64 kernels need twice the registers: 512 */
 #define RES_MAX_THREADS_F64 512
-#define RES_MAX_ATOMS 2047          /* 11-bit neighbour index; slot N_s is the far-away dummy */
+#define RES_MAX_ATOMS 2047          /* builder hit masks cover 8 x 256 candidates */
+#define RES_MAX_SLOTS 4095          /* 16-bit byte offsets of 16-byte slots */
 #define RES_SMEM_LIMIT (227 * 1024)
 
 struct ResCfg {
     int CL;            /* CTAs per system = cluster size                       */
     int A;             /* atoms per CTA, capacity (multiple of 4)              */
     int pitch;         /* u16 entries per list row, pitch mod 64 in {16, 48}   */
-    int NP;            /* max atoms per system + 1                             */
+    int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
-    unsigned posbytes; /* bytes of one position buffer                         */
-    unsigned o_pos, o_fr, o_rows, o_fs, o_cnt, o_shtab, o_pot, o_red, o_cred, o_misc;
+    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc;
     unsigned smem;
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
 };
@@ -63,8 +70,11 @@ struct ResMisc {
     unsigned nnz;
     unsigned rebuilds;
     int overflow;
-    int pad[3];        /* 32 bytes: the fp64 cell copy follows */
+    int pad[3];        /* 32 bytes: the cell copy follows */
 };
+
+__device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 /* ------------------------------------------------------------------ position slots */
 template <typename T> struct P3 { T x, y, z; int ty; };
@@ -123,17 +133,64 @@ __device__ __forceinline__ int row_index(int p)
     return ((k >> 1) << 4) + (l << 1) + (k & 1);
 }
 
-/* ------------------------------------------------------------------ one pair */
-template <typename T, int KIND, bool NT1, bool EV, bool SH>
-__device__ __forceinline__ void pair_accum(const P3<T> &xi, const P3<T> &xj, T sx, T sy, T sz, const PotEntry<T> &pe1,
-                                           const PotEntry<T> *tab, int tirow, T &fx, T &fy, T &fz, T *ev)
+/* ------------------------------------------------------------------ ghosts
+ * gtab entry of an atom: first ghost slot (16 bits) | active axes (3 bits) << 16 | image signs
+ * (bit = 1: the image sits at +h_k) << 19.  The images of an atom are the non-empty subsets m of
+ * its active axes, in increasing m; image number r lives in slot base + 8 r (same bank group). */
+__device__ __forceinline__ int ghost_rank(int m, int act)
+{
+    int idx = 0, p = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        int a = (act >> k) & 1;
+        idx |= (((m >> k) & 1) & a) << p;
+        p += a;
+    }
+    return idx - 1;
+}
+
+/* the owner writes its atom (slot ai) and its ghosts into every CTA of the cluster */
+template <typename T>
+__device__ __forceinline__ void publish_atom(cg::cluster_group &cluster, int CL, unsigned char *posb, unsigned zt, int ai,
+                                             unsigned gdesc, T px, T py, T pz, int ty, const T *gh, bool home, bool ghosts)
+{
+    if (home)
+        for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), (unsigned)ai * 16u, zt, px, py, pz, ty);
+    const int act = (int)(gdesc >> 16) & 7;
+    if (ghosts && act) {
+        const int sg = (int)(gdesc >> 19) & 7;
+        unsigned slot = gdesc & 0xffffu;
+        T a[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            T sgn = ((act >> k) & 1) ? (((sg >> k) & 1) ? (T)1 : (T)-1) : (T)0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) a[k][b] = sgn * gh[3 * k + b];
+        }
+#pragma unroll
+        for (int m = 1; m < 8; ++m) {
+            if ((m & ~act) == 0) {
+                T qx = px, qy = py, qz = pz;
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    if ((m >> k) & 1) { qx += a[k][0]; qy += a[k][1]; qz += a[k][2]; }
+                for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), slot * 16u, zt, qx, qy, qz, ty);
+                slot += 8u;
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ one pair (generic path) */
+template <typename T, int KIND, bool NT1, bool EV>
+__device__ __forceinline__ void pair_accum(const P3<T> &xi, const P3<T> &xj, const PotEntry<T> &pe1, const PotEntry<T> *tab,
+                                           int tirow, T &fx, T &fy, T &fz, T *ev)
 {
     T rx = xj.x - xi.x, ry = xj.y - xi.y, rz = xj.z - xi.z;
-    if (SH) { rx += sx; ry += sy; rz += sz; }
     T r2 = rx * rx + ry * ry + rz * rz;
     PotEntry<T> pe = pe1;
     if (!NT1) pe = tab[tirow + xj.ty];
-    const bool in = r2 < pe.rc2;                 /* strict (R9); the padding dummy sits at 1e15 */
+    const bool in = r2 < pe.rc2;                 /* strict (R9); the padding dummies sit at 1e15 */
     if (EV) {
         T V, g;
         pot_eval<T, KIND>(pe, r2, V, g);
@@ -150,49 +207,97 @@ __device__ __forceinline__ void pair_accum(const P3<T> &xi, const P3<T> &xj, T s
     }
 }
 
-/* Forces of the CTA's own atoms from the shared-memory list; E and W partials into acc8 (fp64). */
+/* ------------------------------------------------------------------ packed fp32 helpers (FFMA2 / FMUL2) */
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+/* Forces of the CTA's own atoms from the shared-memory list; E and W partials into red (fp64).
+ * FAST = fp32 Lennard-Jones, one type, forces only: the two pairs of a lane share packed ops. */
 template <typename T, int KIND, bool NT1, bool EV>
 __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char *posb, const unsigned short *rows,
-                                           const unsigned *cnt, const T *shtab, const PotEntry<T> *tab, T *fs,
-                                           int a_begin, int A_own, int NT, double *red)
+                                           const unsigned *cnt, const PotEntry<T> *tab, T *fs, int a_begin, int A_own,
+                                           int NT, double *red)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
-    const unsigned zt = (unsigned)rc.NP * 16u;
+    const unsigned zt = (unsigned)rc.NS * 16u;
     const int ntasks = (A_own + 3) >> 2;
+    constexpr bool FAST = (sizeof(T) == 4) && KIND == TS_LJ && NT1 && !EV;
     double acc8[EV ? 7 : 1];
     if (EV)
 #pragma unroll
         for (int k = 0; k < 7; ++k) acc8[k] = 0.0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
         T ev[7] = { 0, 0, 0, 0, 0, 0, 0 };
-        int al = task * 4 + q;
-        bool has = al < A_own;
-        int ai = a_begin + (has ? al : 0);
-        P3<T> xi = ld_pos(posb, (unsigned)ai * 16u, zt, (T)0);
-        unsigned c = has ? cnt[al] : 0u;
-        int th2 = (int)(c & 255u) >> 1, ts2 = (int)(c >> 8) >> 1;
+        const int al = task * 4 + q;
+        const bool has = al < A_own;
+        const int ai = a_begin + (has ? al : 0);
+        const P3<T> xi = ld_pos(posb, (unsigned)ai * 16u, zt, (T)0);
+        const int niter = (int)cnt[task];                       /* the same for the four atoms of a task */
         const unsigned *row = (const unsigned *)(rows + (size_t)al * rc.pitch) + l;
-        PotEntry<T> pe1 = tab[NT1 ? 0 : xi.ty * NT];
-        int tirow = xi.ty * NT;
+        const PotEntry<T> pe1 = tab[NT1 ? 0 : xi.ty * NT];
+        const int tirow = xi.ty * NT;
         T fx = 0, fy = 0, fz = 0;
+        if (FAST) {
+            const float xix = (float)xi.x, xiy = (float)xi.y, xiz = (float)xi.z, rc2 = (float)pe1.rc2;
+            const float m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
+            const f32x2 C12 = pk2(m12, m12), C6 = pk2(p6, p6);
+            f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
 #pragma unroll 2
-        for (int k = 0; k < th2; ++k) {
-            unsigned e2 = row[k * 8];
-            P3<T> x0 = ld_pos(posb, e2 & 0xffffu, zt, (T)0);
-            P3<T> x1 = ld_pos(posb, e2 >> 16, zt, (T)0);
-            pair_accum<T, KIND, NT1, EV, false>(xi, x0, (T)0, (T)0, (T)0, pe1, tab, tirow, fx, fy, fz, ev);
-            pair_accum<T, KIND, NT1, EV, false>(xi, x1, (T)0, (T)0, (T)0, pe1, tab, tirow, fx, fy, fz, ev);
-        }
-        row += th2 * 8;
-        for (int k = 0; k < ts2; ++k) {
-            unsigned e2 = row[k * 8];
-            unsigned j0 = (e2 & 0x7ffu) << 4, c0 = (e2 >> 11) & 31u, j1 = ((e2 >> 16) & 0x7ffu) << 4, c1 = e2 >> 27;
-            P3<T> x0 = ld_pos(posb, j0, zt, (T)0);
-            P3<T> x1 = ld_pos(posb, j1, zt, (T)0);
-            const T *s0 = shtab + 4 * c0, *s1 = shtab + 4 * c1;
-            pair_accum<T, KIND, NT1, EV, true>(xi, x0, s0[0], s0[1], s0[2], pe1, tab, tirow, fx, fy, fz, ev);
-            pair_accum<T, KIND, NT1, EV, true>(xi, x1, s1[0], s1[1], s1[2], pe1, tab, tirow, fx, fy, fz, ev);
+            for (int k = 0; k < niter; ++k) {
+                const unsigned e2 = row[k * 8];
+                const float4 pa = *(const float4 *)(posb + (e2 & 0xffffu));
+                const float4 pb = *(const float4 *)(posb + (e2 >> 16));
+                const f32x2 RX = pk2(pa.x - xix, pb.x - xix), RY = pk2(pa.y - xiy, pb.y - xiy), RZ = pk2(pa.z - xiz, pb.z - xiz);
+                f32x2 R2 = mul2(RX, RX);
+                R2 = fma2(RY, RY, R2);
+                R2 = fma2(RZ, RZ, R2);
+                float r2a, r2b;
+                upk2(R2, r2a, r2b);
+                float ia, ib;
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
+                const float ma = r2a < rc2 ? 1.0f : 0.0f, mb = r2b < rc2 ? 1.0f : 0.0f;   /* strict (R9) */
+                const f32x2 I = mul2(pk2(ia, ib), pk2(ma, mb));
+                const f32x2 I2 = mul2(I, I);
+                const f32x2 I6 = mul2(I2, I);
+                const f32x2 P = fma2(I6, C12, C6);
+                const f32x2 G = mul2(mul2(I6, I), P);              /* g = V'(r)/r = ir2 ir6 (6 c1 - 12 c0 ir6) */
+                FX = fma2(G, RX, FX);
+                FY = fma2(G, RY, FY);
+                FZ = fma2(G, RZ, FZ);
+            }
+            float a, b;
+            upk2(FX, a, b); fx = (T)(a + b);
+            upk2(FY, a, b); fy = (T)(a + b);
+            upk2(FZ, a, b); fz = (T)(a + b);
+        } else {
+#pragma unroll 2
+            for (int k = 0; k < niter; ++k) {
+                const unsigned e2 = row[k * 8];
+                const P3<T> x0 = ld_pos(posb, e2 & 0xffffu, zt, (T)0);
+                const P3<T> x1 = ld_pos(posb, e2 >> 16, zt, (T)0);
+                pair_accum<T, KIND, NT1, EV>(xi, x0, pe1, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x1, pe1, tab, tirow, fx, fy, fz, ev);
+            }
         }
 #pragma unroll
         for (int o = 1; o < 8; o <<= 1) {
@@ -200,11 +305,13 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char
             fy += __shfl_xor_sync(0xffffffffu, fy, o);
             fz += __shfl_xor_sync(0xffffffffu, fz, o);
         }
-        if (has && l == 0) { fs[al] = fx; fs[rc.A + al] = fy; fs[2 * rc.A + al] = fz; }
+        if (has && l < 3) fs[l * rc.A + al] = l == 0 ? fx : (l == 1 ? fy : fz);
         if (EV) {                       /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
-            acc8[0] += 0.5 * (double)ev[0];
+            if (has) {
+                acc8[0] += 0.5 * (double)ev[0];
 #pragma unroll
-            for (int k = 1; k < 7; ++k) acc8[k] += -0.5 * (double)ev[k];
+                for (int k = 1; k < 7; ++k) acc8[k] += -0.5 * (double)ev[k];
+            }
         }
     }
     if (EV) {                           /* warp partials of E, W into red[warp][0..6] */
@@ -217,96 +324,130 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char
     }
 }
 
+/* ------------------------------------------------------------------ ghost table (identical in every CTA) */
+/* thr[k] = fixed-point fraction within which an atom is close enough to a face to need an image */
+__device__ __forceinline__ void ghost_table(const ResCfg &rc, const uint4 *fr, unsigned *gtab, const unsigned *thr, int N_s,
+                                            int NSB, ResMisc *misc)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int j = threadIdx.x; j < N_s; j += blockDim.x) {
+        const uint4 u = fr[j];
+        const unsigned uu[3] = { u.x, u.y, u.z };
+        unsigned act = 0u, sg = 0u;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const bool lo = uu[k] < thr[k], hi = uu[k] > ~thr[k];
+            act |= (unsigned)(lo || hi) << k;
+            sg |= (unsigned)(uu[k] < 0x80000000u) << k;
+        }
+        gtab[j] = (act << 16) | (sg << 19) | ((1u << __popc(act)) - 1u);          /* low bits: image count for now */
+    }
+    __syncthreads();
+    if (warp < 8) {                               /* warp g scans the atoms j = g mod 8: slots stay in bank group g */
+        const int g = warp;
+        unsigned run = 0u;
+        for (int j0 = g; j0 < N_s; j0 += 256) {
+            const int j = j0 + 8 * lane;
+            const unsigned e = j < N_s ? gtab[j] : 0u;
+            const unsigned c = e & 0xffffu;
+            unsigned inc = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned v = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += v;
+            }
+            const unsigned slot = (unsigned)NSB + 8u * (run + inc - c) + (unsigned)g;
+            if (j < N_s) gtab[j] = (e & 0xffff0000u) | (slot & 0xffffu);
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (lane == 0 && (unsigned)NSB + 8u * run + 8u > (unsigned)rc.NS) misc->overflow = 1;   /* more images than planned */
+    }
+    __syncthreads();
+}
+
 /* ------------------------------------------------------------------ list build (per CTA, own atoms) */
 /* One quarter-warp per atom; lane l tests the candidates j = l mod 8 (bank group l), keeps the hits
  * as a bit mask in registers, then places its hits in round-robin order (rr_position).            */
-__device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, unsigned short *rows, unsigned *cnt,
-                                            const float *G, float rb2, int a_begin, int A_own, int N_s, ResMisc *misc)
+__device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, const unsigned *gtab, unsigned short *rows,
+                                            unsigned *cnt, const float *G, float rb2, int a_begin, int A_own, int N_s,
+                                            int N8, ResMisc *misc)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
     const int ntasks = (A_own + 3) >> 2;
     const float G0 = G[0], G1 = G[1], G2 = G[2], G3 = G[3], G4 = G[4], G5 = G[5];
+    const bool ovf = misc->overflow != 0;         /* ghost slots exhausted: leave every row empty (flagged) */
     unsigned nnz = 0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
-        int al = task * 4 + q;
-        bool has = al < A_own;
-        int ai = a_begin + (has ? al : 0);
-        uint4 ui = fr[ai];
+        const int al = task * 4 + q;
+        const bool has = al < A_own;
+        const int ai = a_begin + (has ? al : 0);
+        const uint4 ui = fr[ai];
         unsigned mask[8];
+        int mine = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
             unsigned word = 0u;
-            if (w * 256 < N_s) {
-                int jb = w * 256 + l;
+            if (has && w * 256 < N_s) {
+                const int jb = w * 256 + l;
 #pragma unroll 4
                 for (int b = 0; b < 32; ++b) {
-                    int j = jb + b * 8;
+                    const int j = jb + b * 8;
                     if (j < N_s) {
-                        uint4 uj = fr[j];
-                        float e0 = (float)(int)(uj.x - ui.x), e1 = (float)(int)(uj.y - ui.y), e2 = (float)(int)(uj.z - ui.z);
-                        float r2 = e0 * (G0 * e0 + G1 * e1 + G2 * e2) + e1 * (G3 * e1 + G4 * e2) + G5 * e2 * e2;
+                        const uint4 uj = fr[j];
+                        const float e0 = (float)(int)(uj.x - ui.x), e1 = (float)(int)(uj.y - ui.y), e2 = (float)(int)(uj.z - ui.z);
+                        const float r2 = e0 * (G0 * e0 + G1 * e1 + G2 * e2) + e1 * (G3 * e1 + G4 * e2) + G5 * e2 * e2;
                         if (r2 < rb2 && j != ai) word |= 1u << b;
                     }
                 }
             }
             mask[w] = word;
+            mine += __popc(word);
         }
-        /* classify my hits: home (shift 0) or shifted */
-        int nh = 0, ns = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) {
-            unsigned word = mask[w];
-            while (word) {
-                int b = __ffs(word) - 1;
-                word &= word - 1u;
-                uint4 uj = fr[w * 256 + b * 8 + l];
-                int sh = image_shift(uj.x, ui.x) | image_shift(uj.y, ui.y) | image_shift(uj.z, ui.z);
-                if (sh) ns += 1; else nh += 1;
-            }
-        }
-        int cH[8], cS[8], NH = 0, NS = 0;
+        int c[8], NT = 0;
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
-            cH[g] = __shfl_sync(0xffffffffu, nh, (lane & 24) | g);
-            cS[g] = __shfl_sync(0xffffffffu, ns, (lane & 24) | g);
-            NH += cH[g]; NS += cS[g];
+            c[g] = __shfl_sync(0xffffffffu, mine, (lane & 24) | g);
+            NT += c[g];
         }
-        int th = ((NH + 15) >> 4) << 1, tsn = ((NS + 15) >> 4) << 1;      /* k counts, even */
-        bool fits = 8 * (th + tsn) <= rc.pitch && th < 256 && tsn < 256;
+        int niter = (NT + 15) >> 4;                                 /* u32 per lane: 16 entries per iteration */
+        niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 8));
+        niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16)); /* the four atoms of a task share the loop count */
+        const bool fits = 16 * niter <= rc.pitch && !ovf;
         if (!fits) {
-            if (has) misc->overflow = 1;
-            th = 0; tsn = 0;
+            if (lane == 0) misc->overflow = 1;
+            niter = 0;
         }
         unsigned short *row = rows + (size_t)al * rc.pitch;
-        if (has && fits) {
-            int mh = 0, ms = 0;
+        if (fits) {
+            int m = 0;
 #pragma unroll
             for (int w = 0; w < 8; ++w) {
                 unsigned word = mask[w];
                 while (word) {
-                    int b = __ffs(word) - 1;
+                    const int b = __ffs(word) - 1;
                     word &= word - 1u;
-                    int j = w * 256 + b * 8 + l;
-                    uint4 uj = fr[j];
-                    int s0 = image_shift(uj.x, ui.x), s1 = image_shift(uj.y, ui.y), s2 = image_shift(uj.z, ui.z);
-                    if ((s0 | s1 | s2) == 0) {
-                        row[row_index(rr_position(cH, l, mh))] = (unsigned short)(j << 4);
-                        mh += 1;
-                    } else {
-                        int code = (s0 + 1) * 9 + (s1 + 1) * 3 + (s2 + 1);
-                        row[row_index(8 * th + rr_position(cS, l, ms))] = (unsigned short)(j | (code << 11));
-                        ms += 1;
+                    const int j = w * 256 + b * 8 + l;
+                    const uint4 uj = fr[j];
+                    const int s0 = image_shift(uj.x, ui.x), s1 = image_shift(uj.y, ui.y), s2 = image_shift(uj.z, ui.z);
+                    unsigned slot = (unsigned)j;
+                    if ((s0 | s1 | s2) != 0) {
+                        const unsigned gd = gtab[j];
+                        const int act = (int)(gd >> 16) & 7, sg = (int)(gd >> 19) & 7;
+                        const int mm = (s0 != 0) | ((s1 != 0) << 1) | ((s2 != 0) << 2);
+                        const int want = (s0 > 0) | ((s1 > 0) << 1) | ((s2 > 0) << 2);
+                        if ((mm & ~act) != 0 || ((sg ^ want) & mm) != 0) misc->overflow = 1;   /* cannot happen: see ghost_table */
+                        slot = (gd & 0xffffu) + 8u * (unsigned)ghost_rank(mm, act);
                     }
+                    row[row_index(rr_position(c, l, m))] = (unsigned short)(slot << 4);
+                    m += 1;
                 }
             }
-            for (int p = NH + l; p < 8 * th; p += 8) row[row_index(p)] = (unsigned short)(N_s << 4);
-            for (int p = NS + l; p < 8 * tsn; p += 8) row[row_index(8 * th + p)] = (unsigned short)(N_s | (13 << 11));
+            /* padding: lane l owns the positions p = l mod 8 and pads them with the dummy of its bank group */
+            for (int p = NT + ((l - NT) & 7); p < 16 * niter; p += 8) row[row_index(p)] = (unsigned short)((N8 + l) << 4);
         }
-        if (has && l == 0) {
-            cnt[al] = (unsigned)th | ((unsigned)tsn << 8);
-            nnz += (unsigned)(NH + NS);
-        }
+        if (lane == 0) cnt[task] = (unsigned)niter;
+        if (has && l == 0) nnz += (unsigned)NT;
     }
     if (nnz) atomicAdd(&misc->nnz, nnz);
 }
@@ -345,20 +486,21 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     const int rank = (int)cluster.block_rank();
     const int cid = (int)(blockIdx.x / (unsigned)CL);
     const int tid = threadIdx.x;
-    const unsigned zt = (unsigned)rc.NP * 16u;
+    const unsigned zt = (unsigned)rc.NS * 16u;
 
-    unsigned char *const posb0 = smem + rc.o_pos, *const posb1 = smem + rc.o_pos + rc.posbytes;
+    unsigned char *const posb = smem + rc.o_pos;
     uint4 *fr = (uint4 *)(smem + rc.o_fr);
+    unsigned *gtab = (unsigned *)(smem + rc.o_gtab);
     unsigned short *rows = (unsigned short *)(smem + rc.o_rows);
     T *fs = (T *)(smem + rc.o_fs);
     unsigned *cnt = (unsigned *)(smem + rc.o_cnt);
-    T *shtab = (T *)(smem + rc.o_shtab);
     PotEntry<T> *tab = (PotEntry<T> *)(smem + rc.o_pot);
     double *red = (double *)(smem + rc.o_red);
     double *cred = (double *)(smem + rc.o_cred);
     ResMisc *misc = (ResMisc *)(smem + rc.o_misc);
     T *gh = (T *)(misc + 1);            /* h[9], hinv[9] in the state dtype */
     float *G = (float *)(gh + 18);      /* metric of the fixed-point fractions, [6] + rb2 */
+    unsigned *thr = (unsigned *)(G + 8);/* ghost thresholds [3] */
 
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
@@ -366,18 +508,13 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     for (int s = cid; s < d.S; s += rc.n_clusters) {
         const int g0 = d.sysoff[s];
         const int N_s = d.sysoff[s + 1] - g0;
+        const int N8 = (N_s + 7) & ~7;
         const int A_s = ((((N_s + CL - 1) / CL) + 3) >> 2) << 2;
         const int a_begin = rank * A_s;
         const int A_own = max(0, min(A_s, N_s - a_begin));
         const SysGeom &geo = d.geom[s];
         /* ---- per-system constants into shared memory */
         if (tid < 9) { gh[tid] = (T)geo.h[tid]; gh[9 + tid] = (T)geo.hinv[tid]; }
-        if (tid >= 32 && tid < 32 + 27) {
-            int code = tid - 32;
-            double s0 = (double)(code / 9 - 1), s1 = (double)((code / 3) % 3 - 1), s2 = (double)(code % 3 - 1);
-            for (int b = 0; b < 3; ++b) shtab[4 * code + b] = (T)(s0 * geo.h[b] + s1 * geo.h[3 + b] + s2 * geo.h[6 + b]);
-            shtab[4 * code + 3] = (T)0;
-        }
         if (tid == 64) {
             const double *h = geo.h;
             double M[6], lmax = 0.0;
@@ -390,8 +527,12 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             const double sc = 1.0 / 18446744073709551616.0;      /* 2^-64 */
             for (int e = 0; e < 6; ++e) G[e] = (float)(M[e] * sc);
             for (int a = 0; a < 3; ++a) lmax = fmax(lmax, sqrt(h[3 * a] * h[3 * a] + h[3 * a + 1] * h[3 * a + 1] + h[3 * a + 2] * h[3 * a + 2]));
-            double rb = d.r_list + (double)rc.eps_rel * lmax;
+            const double rb = d.r_list + (double)rc.eps_rel * lmax;
             G[6] = (float)(rb * rb);
+            for (int k = 0; k < 3; ++k) {       /* a pair within rb that wraps along k has u_j within rb / h_perp of a face */
+                double rho = (rb + 2.0 * (double)rc.eps_rel * lmax) / geo.hperp[k] + 1e-6;
+                thr[k] = rho >= 0.5 ? 0x80000000u : (unsigned)(rho * 4294967296.0);
+            }
             misc->flags[0] = 0; misc->flags[1] = 0; misc->nnz = 0u; misc->rebuilds = 0u; misc->overflow = 0;
         }
         /* ---- owner state */
@@ -401,6 +542,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         T x0 = 0, x1 = 0, x2 = 0, v0 = 0, v1 = 0, v2 = 0, f0 = 0, f1 = 0, f2 = 0, r0 = 0, r1 = 0, r2 = 0;
         T ws0 = 0, ws1 = 0, ws2 = 0, im = 0, mass = 0;
         int ty = 0;
+        unsigned gdesc = 0u;
         if (own) {
             const T *x = (const T *)d.pos + 3 * gi, *v = (const T *)d.vel + 3 * gi;
             x0 = x[0]; x1 = x[1]; x2 = x[2]; v0 = v[0]; v1 = v[1]; v2 = v[2];
@@ -415,35 +557,38 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
 
         for (int n = 0; n <= n_steps; ++n) {
             const int nb = n & 1;
-            unsigned char *const posn = nb ? posb1 : posb0;
-            bool moved = false;
-            if (n > 0 && own) {
-                /* first half of the step (O3 / O4), as in the general engine */
-                if (c.integrator == TS_NVE) {
-                    v0 = v0 + hdt * (f0 * im); x0 = x0 + dt * v0;
-                    v1 = v1 + hdt * (f1 * im); x1 = x1 + dt * v1;
-                    v2 = v2 + hdt * (f2 * im); x2 = x2 + dt * v2;
-                } else {
-                    unsigned long long step = step0 + (unsigned long long)(n - 1);
-                    unsigned w[4];
-                    philox4x32_10((unsigned)ai, uid, (unsigned)(step & 0xffffffffull), (unsigned)(step >> 32), c.key0, c.key1, w);
-                    T xi[3];
-                    normals3(w, xi);
-                    T sig = sizeof(T) == 4 ? (T)sqrtf((float)((T)c.kT * im)) : (T)sqrt((double)((T)c.kT * im));
-                    T c1 = (T)c.c1, c2 = (T)c.c2;
-                    v0 = v0 + hdt * (f0 * im); x0 = x0 + hdt * v0; v0 = c1 * v0 + c2 * sig * xi[0]; x0 = x0 + hdt * v0;
-                    v1 = v1 + hdt * (f1 * im); x1 = x1 + hdt * v1; v1 = c1 * v1 + c2 * sig * xi[1]; x1 = x1 + hdt * v1;
-                    v2 = v2 + hdt * (f2 * im); x2 = x2 + hdt * v2; v2 = c1 * v2 + c2 * sig * xi[2]; x2 = x2 + hdt * v2;
+            if (n > 0) {
+                bool moved = false;
+                if (own) {
+                    /* first half of the step (O3 / O4), as in the general engine */
+                    if (c.integrator == TS_NVE) {
+                        v0 = v0 + hdt * (f0 * im); x0 = x0 + dt * v0;
+                        v1 = v1 + hdt * (f1 * im); x1 = x1 + dt * v1;
+                        v2 = v2 + hdt * (f2 * im); x2 = x2 + dt * v2;
+                    } else {
+                        unsigned long long step = step0 + (unsigned long long)(n - 1);
+                        unsigned w[4];
+                        philox4x32_10((unsigned)ai, uid, (unsigned)(step & 0xffffffffull), (unsigned)(step >> 32), c.key0, c.key1, w);
+                        T xi[3];
+                        normals3(w, xi);
+                        T sig = sizeof(T) == 4 ? (T)sqrtf((float)((T)c.kT * im)) : (T)sqrt((double)((T)c.kT * im));
+                        T c1 = (T)c.c1, c2 = (T)c.c2;
+                        v0 = v0 + hdt * (f0 * im); x0 = x0 + hdt * v0; v0 = c1 * v0 + c2 * sig * xi[0]; x0 = x0 + hdt * v0;
+                        v1 = v1 + hdt * (f1 * im); x1 = x1 + hdt * v1; v1 = c1 * v1 + c2 * sig * xi[1]; x1 = x1 + hdt * v1;
+                        v2 = v2 + hdt * (f2 * im); x2 = x2 + hdt * v2; v2 = c1 * v2 + c2 * sig * xi[2]; x2 = x2 + hdt * v2;
+                    }
+                    T a = x0 - r0, b = x1 - r1, cc = x2 - r2;
+                    moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
                 }
-                T a = x0 - r0, b = x1 - r1, cc = x2 - r2;
-                moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
-                for (int r = 0; r < CL; ++r) {
-                    unsigned char *pb = cluster.map_shared_rank(posn, r);
-                    st_pos(pb, (unsigned)ai * 16u, zt, x0 - ws0, x1 - ws1, x2 - ws2, ty);
-                    if (moved) cluster.map_shared_rank(misc, r)->flags[nb] = 1;
+                cl_wait();                            /* every CTA of the cluster has finished reading the old positions */
+                if (own) {
+                    if (moved)
+                        for (int r = 0; r < CL; ++r) cluster.map_shared_rank(misc, r)->flags[nb] = 1;
+                    publish_atom<T>(cluster, CL, posb, zt, ai, gdesc, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, true, true);
                 }
+                cl_arrive();
+                cl_wait();                            /* new positions (and the rebuild flag) visible everywhere */
             }
-            if (n > 0) cluster.sync();
             const bool rebuild = (n == 0) || (misc->flags[nb] != 0);
             if (rebuild) {
                 __syncthreads();
@@ -462,31 +607,35 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     ws1 = wa * gh[1] + wb * gh[4] + wc * gh[7];
                     ws2 = wa * gh[2] + wb * gh[5] + wc * gh[8];
                     r0 = x0; r1 = x1; r2 = x2;
-                    uint4 u = make_uint4(frac_to_u32(fa), frac_to_u32(fb), frac_to_u32(fc), 0u);
-                    for (int r = 0; r < CL; ++r) {
-                        unsigned char *pb = cluster.map_shared_rank(posn, r);
-                        st_pos(pb, (unsigned)ai * 16u, zt, x0 - ws0, x1 - ws1, x2 - ws2, ty);
-                        cluster.map_shared_rank(fr, r)[ai] = u;
-                    }
+                    const uint4 u = make_uint4(frac_to_u32(fa), frac_to_u32(fb), frac_to_u32(fc), 0u);
+                    for (int r = 0; r < CL; ++r) cluster.map_shared_rank(fr, r)[ai] = u;
+                    publish_atom<T>(cluster, CL, posb, zt, ai, 0u, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, true, false);
                 }
-                if (tid == 0) {                       /* the far-away dummy neighbour (list padding), both buffers */
-                    T far = (T)1e15;
-                    st_pos(posb0, (unsigned)N_s * 16u, zt, far, far, far, 0);
-                    st_pos(posb1, (unsigned)N_s * 16u, zt, far, far, far, 0);
+                if (tid < 8) {                        /* the far-away dummy neighbours (list padding), one per bank group */
+                    const T far = (T)1e15;
+                    st_pos(posb, (unsigned)(N8 + tid) * 16u, zt, far, far, far, 0);
                 }
-                cluster.sync();
-                build_phase(rc, fr, rows, cnt, G, G[6], a_begin, A_own, N_s, misc);
+                cluster.sync();                       /* fractions and home slots complete in every CTA */
+                ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
+                if (own) {
+                    gdesc = misc->overflow ? 0u : gtab[ai];   /* on overflow (flagged) nothing is written past the slots */
+                    publish_atom<T>(cluster, CL, posb, zt, ai, gdesc, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, false, true);
+                }
+                cluster.sync();                       /* ghost slots complete in every CTA */
+                build_phase(rc, fr, gtab, rows, cnt, G, G[6], a_begin, A_own, N_s, N8, misc);
                 __syncthreads();
             }
             const bool last = n == n_steps;
-            if (last) pair_phase<T, KIND, NT1, true>(rc, posn, rows, cnt, shtab, tab, fs, a_begin, A_own, NT, red);
-            else pair_phase<T, KIND, NT1, false>(rc, posn, rows, cnt, shtab, tab, fs, a_begin, A_own, NT, red);
+            if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
+            else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
+            cl_arrive();                              /* this CTA no longer reads the positions of step n */
             __syncthreads();
             if (own) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
                 if (n > 0) { v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im); }
             }
         }
+        cl_wait();                                    /* pairs the last arrive */
         /* ---- store the system (R16): x, v at t + n dt, F(x), E, W, KE */
         double ke = 0.0;
         if (own) {
@@ -544,31 +693,31 @@ static ResKernel pick_kernel(const ts_state *st)
 static unsigned up16(unsigned x) { return (x + 15u) & ~15u; }
 
 /* Shared-memory carve for cluster size CL; returns false when it does not fit. */
-static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int dtype, int n_types)
+static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types)
 {
     size_t w = dtype == TS_F32 ? 4 : 8;
     int A = ((((nmax + CL - 1) / CL) + 3) / 4) * 4;
     const int max_threads = dtype == TS_F32 ? RES_MAX_THREADS : RES_MAX_THREADS_F64;
     if (A > max_threads) return false;
-    int pitch = 32 * ((need_row - 16 + 31) / 32) + 16;
+    int pitch = 32 * ((need_row - 16 + 31) / 32) + 16;           /* multiple of 16, rows 32 bytes apart modulo 128 */
     if (pitch < 48) pitch = 48;
     int ntasks = A / 4, maxw = max_threads / 32;
     int passes = (ntasks + maxw - 1) / maxw;
     int nwarps = (ntasks + passes - 1) / passes;
     if (nwarps * 32 < A) nwarps = (A + 31) / 32;
-    c.CL = CL; c.A = A; c.pitch = pitch; c.NP = nmax + 1; c.nwarps = nwarps;
-    c.posbytes = up16((unsigned)(c.NP * 4 * w));
+    if (nwarps < 8) nwarps = 8;                                   /* ghost_table scans with eight warps */
+    c.CL = CL; c.A = A; c.pitch = pitch; c.NS = need_slots; c.nwarps = nwarps;
     unsigned o = 0;
-    c.o_pos = o; o += 2 * c.posbytes;
-    c.o_fr = o; o += up16((unsigned)c.NP * 16u);
+    c.o_pos = o; o += up16((unsigned)(c.NS * 4 * w));
+    c.o_fr = o; o += up16((unsigned)nmax * 16u);
+    c.o_gtab = o; o += up16((unsigned)nmax * 4u);
     c.o_rows = o; o += up16((unsigned)A * (unsigned)pitch * 2u);
     c.o_fs = o; o += up16((unsigned)(3 * A * w));
     c.o_cnt = o; o += up16((unsigned)A * 4u);
-    c.o_shtab = o; o += up16((unsigned)(27 * 4 * w));
     c.o_pot = o; o += up16((unsigned)(n_types * n_types * (dtype == TS_F32 ? sizeof(PotEntry<float>) : sizeof(PotEntry<double>))));
     c.o_red = o; o += (unsigned)(RES_MAX_THREADS / 32) * 64u;
     c.o_cred = o; o += 8u * 64u;
-    c.o_misc = o; o += up16((unsigned)(sizeof(ResMisc) + 18 * w + 8 * sizeof(float)));
+    c.o_misc = o; o += up16((unsigned)(sizeof(ResMisc) + 18 * w + 8 * sizeof(float) + 4 * sizeof(unsigned)));
     c.smem = o;
     return o <= RES_SMEM_LIMIT;
 }
@@ -586,7 +735,7 @@ bool resident_supported(ts_state *st)
     if (cudaMemcpy(geo.data(), d.geom, sizeof(SysGeom) * (size_t)S, cudaMemcpyDeviceToHost) != cudaSuccess) return false;
     const float eps_rel = 4e-6f;
     int nmax = 0;
-    double need = 0.0;
+    double need = 0.0, need_slots = 0.0;
     for (int s = 0; s < S; ++s) {
         int n = st->h_sysoff[s + 1] - st->h_sysoff[s];
         nmax = n > nmax ? n : nmax;
@@ -594,15 +743,24 @@ bool resident_supported(ts_state *st)
         double lmax = 0.0;
         for (int a = 0; a < 3; ++a)
             lmax = fmax(lmax, sqrt(g.h[3 * a] * g.h[3 * a] + g.h[3 * a + 1] * g.h[3 * a + 1] + g.h[3 * a + 2] * g.h[3 * a + 2]));
-        double rb = d.r_list + 2.0 * eps_rel * lmax;
-        for (int k = 0; k < 3; ++k)
+        double rb = d.r_list + 4.0 * eps_rel * lmax;
+        double images = 1.0;
+        for (int k = 0; k < 3; ++k) {
             if (!(g.hperp[k] >= 2.0 * rb)) return false;          /* more than one image within r_list possible */
+            images *= 1.0 + fmin(1.0, 2.0 * rb / g.hperp[k]);
+        }
         double nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
         need = fmax(need, nbar);
+        /* atoms + dummies + expected ghosts (uniform density) with 25 % head room; 8 more per bank group for the
+         * uneven fill of the eight per-group slot sequences */
+        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 1.25 * (images - 1.0) * n + 8.0 * 16.0);
     }
     if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
+    int ns = (((int)ceil(need_slots) + 7) / 8) * 8;
+    if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
+    if (ns < ((nmax + 7) & ~7) + 16) return false;
     double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
-    int need_row = (int)ceil(need * slack) + 40;                   /* + padding of both segments to 16 */
+    int need_row = (int)ceil(need * slack) + 16;                   /* + padding to 16 */
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -610,7 +768,7 @@ bool resident_supported(ts_state *st)
     for (int CL = 1; CL <= 8; CL *= 2) {
         ResCfg c;
         memset(&c, 0, sizeof c);
-        if (!res_layout(c, CL, nmax, need_row, d.dtype, d.n_types)) continue;
+        if (!res_layout(c, CL, nmax, need_row, ns, d.dtype, d.n_types)) continue;
         best = c; have = true;
         if ((long long)S * CL >= (nsm * 3) / 4 || c.A <= 64) break;   /* enough CTAs to occupy the chip */
     }
