@@ -38,6 +38,7 @@
 #include <cooperative_groups.h>
 #include <math.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <vector>
 
@@ -72,6 +73,14 @@ struct ResMisc {
     int overflow;
     int pad[3];        /* 32 bytes: the cell copy follows */
 };
+
+/* optional phase timers (build with -DTS_RES_TIMING; debugging only): cycles of warp 0 of every CTA */
+#ifdef TS_RES_TIMING
+__device__ unsigned long long g_res_prof[16];
+#define TICK(k) do { if (threadIdx.x == 0) { long long t__ = clock64(); prof_acc[k] += t__ - prof_t; prof_t = t__; } } while (0)
+#else
+#define TICK(k) do { } while (0)
+#endif
 
 __device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
@@ -109,23 +118,6 @@ template <typename T> __device__ __forceinline__ T t_floor(T x);
 template <> __device__ __forceinline__ float t_floor<float>(float x) { return floorf(x); }
 template <> __device__ __forceinline__ double t_floor<double>(double x) { return floor(x); }
 
-/* image shift of j relative to i in one direction from the fixed-point fractions */
-__device__ __forceinline__ int image_shift(unsigned uj, unsigned ui)
-{
-    int dd = (int)(uj - ui);
-    return (uj > ui && dd < 0) ? -1 : ((uj < ui && dd > 0) ? 1 : 0);
-}
-
-/* position p of the m-th member of bank group g in the round-robin order over groups with
- * populations c[0..7]: all members of rank < m first, then the groups below g that reach rank m */
-__device__ __forceinline__ int rr_position(const int c[8], int g, int m)
-{
-    int p = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) p += min(c[k], m) + ((k < g && c[k] > m) ? 1 : 0);
-    return p;
-}
-
 /* u16 index of list slot p (p = 8 k + lane) inside a row: pairs of k interleaved per lane */
 __device__ __forceinline__ int row_index(int p)
 {
@@ -136,46 +128,47 @@ __device__ __forceinline__ int row_index(int p)
 /* ------------------------------------------------------------------ ghosts
  * gtab entry of an atom: first ghost slot (16 bits) | active axes (3 bits) << 16 | image signs
  * (bit = 1: the image sits at +h_k) << 19.  The images of an atom are the non-empty subsets m of
- * its active axes, in increasing m; image number r lives in slot base + 8 r (same bank group). */
-__device__ __forceinline__ int ghost_rank(int m, int act)
+ * its active axes, in increasing m; image number r lives in slot base + 8 r (same bank group as
+ * the atom).  Owners publish only the HOME slot of their atom through DSMEM; every CTA then
+ * regenerates all ghost slots locally from its home slots (ghost_pass, one thread per atom): DSMEM
+ * carries 16 bytes per atom and peer instead of 16 bytes per image.                               */
+
+/* the owner writes the home slot of its atom into every CTA of the cluster */
+template <typename T>
+__device__ __forceinline__ void publish_home(cg::cluster_group &cluster, int CL, unsigned char *posb, unsigned zt, int ai,
+                                             T px, T py, T pz, int ty)
 {
-    int idx = 0, p = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        int a = (act >> k) & 1;
-        idx |= (((m >> k) & 1) & a) << p;
-        p += a;
-    }
-    return idx - 1;
+    for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), (unsigned)ai * 16u, zt, px, py, pz, ty);
 }
 
-/* the owner writes its atom (slot ai) and its ghosts into every CTA of the cluster */
+/* every CTA refreshes the images of every atom of the system from the home slots */
 template <typename T>
-__device__ __forceinline__ void publish_atom(cg::cluster_group &cluster, int CL, unsigned char *posb, unsigned zt, int ai,
-                                             unsigned gdesc, T px, T py, T pz, int ty, const T *gh, bool home, bool ghosts)
+__device__ __forceinline__ void ghost_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int N_s)
 {
-    if (home)
-        for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), (unsigned)ai * 16u, zt, px, py, pz, ty);
-    const int act = (int)(gdesc >> 16) & 7;
-    if (ghosts && act) {
-        const int sg = (int)(gdesc >> 19) & 7;
-        unsigned slot = gdesc & 0xffffu;
+    for (int j = threadIdx.x; j < N_s; j += (int)blockDim.x) {
+        const unsigned e = gtab[j];
+        const unsigned act = (e >> 16) & 7u;
+        if (act == 0u) continue;
+        const P3<T> p = ld_pos(posb, (unsigned)j * 16u, zt, (T)0);
         T a[3][3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            T sgn = ((act >> k) & 1) ? (((sg >> k) & 1) ? (T)1 : (T)-1) : (T)0;
+            const T sgn = ((e >> (19 + k)) & 1u) ? (T)1 : (T)-1;
 #pragma unroll
             for (int b = 0; b < 3; ++b) a[k][b] = sgn * gh[3 * k + b];
         }
+        /* q[m] = p + sum_{k in m} a_k, built incrementally: q[m] = q[m without its top axis] + a_top */
+        T q[8][3] = { { p.x, p.y, p.z } };
+        unsigned off = (e & 0xffffu) * 16u;
 #pragma unroll
         for (int m = 1; m < 8; ++m) {
-            if ((m & ~act) == 0) {
-                T qx = px, qy = py, qz = pz;
+            const int top = m >= 4 ? 2 : (m >= 2 ? 1 : 0);
+            const int rest = m & ~(1 << top);
 #pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    if ((m >> k) & 1) { qx += a[k][0]; qy += a[k][1]; qz += a[k][2]; }
-                for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), slot * 16u, zt, qx, qy, qz, ty);
-                slot += 8u;
+            for (int b = 0; b < 3; ++b) q[m][b] = q[rest][b] + a[top][b];
+            if ((m & ~act) == 0u) {
+                st_pos(posb, off, zt, q[m][0], q[m][1], q[m][2], p.ty);
+                off += 128u;
             }
         }
     }
@@ -363,11 +356,25 @@ __device__ __forceinline__ void ghost_table(const ResCfg &rc, const uint4 *fr, u
         if (lane == 0 && (unsigned)NSB + 8u * run + 8u > (unsigned)rc.NS) misc->overflow = 1;   /* more images than planned */
     }
     __syncthreads();
+    /* flagged overflow: no atom gets an image (and build_phase leaves every row empty) */
+    if (misc->overflow)
+        for (int j = threadIdx.x; j < N_s; j += blockDim.x) gtab[j] = 0u;
+    __syncthreads();
 }
 
 /* ------------------------------------------------------------------ list build (per CTA, own atoms) */
-/* One quarter-warp per atom; lane l tests the candidates j = l mod 8 (bank group l), keeps the hits
- * as a bit mask in registers, then places its hits in round-robin order (rr_position).            */
+/* One quarter-warp per atom; lane l tests the candidates j = 8 t + l (bank group l) and keeps the
+ * hits as bit t of a mask in registers.  Two candidates per loop trip share packed f32x2 ops.  The
+ * fractions fr[] are padded to a multiple of 16 atoms, so the loop carries no bounds checks; the
+ * bits of j >= N_s and of j == i are cleared afterwards.                                          */
+__device__ __forceinline__ unsigned wrap_bit(unsigned uj, unsigned ui)
+{
+    /* bit 31 = 1 when the minimum image of j relative to i along this axis is not the home image:
+     * borrow(uj - ui) xor sign(uj - ui), one LOP3 */
+    const unsigned dd = uj - ui;
+    return (((~uj & ui) | (~(uj ^ ui) & dd)) ^ dd) >> 31;
+}
+
 __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, const unsigned *gtab, unsigned short *rows,
                                             unsigned *cnt, const float *G, float rb2, int a_begin, int A_own, int N_s,
                                             int N8, ResMisc *misc)
@@ -375,8 +382,11 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
     const int ntasks = (A_own + 3) >> 2;
-    const float G0 = G[0], G1 = G[1], G2 = G[2], G3 = G[3], G4 = G[4], G5 = G[5];
+    const f32x2 G0 = pk2(G[0], G[0]), G1 = pk2(G[1], G[1]), G2 = pk2(G[2], G[2]);
+    const f32x2 G3 = pk2(G[3], G[3]), G4 = pk2(G[4], G[4]), G5 = pk2(G[5], G[5]);
     const bool ovf = misc->overflow != 0;         /* ghost slots exhausted: leave every row empty (flagged) */
+    const int T = (N_s + 7) >> 3;                 /* candidates per lane */
+    const int W = (T + 31) >> 5;                  /* mask words per lane */
     unsigned nnz = 0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
         const int al = task * 4 + q;
@@ -388,28 +398,42 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
             unsigned word = 0u;
-            if (has && w * 256 < N_s) {
-                const int jb = w * 256 + l;
+            if (w < W) {
+                const uint4 *cj = fr + (w * 256 + l);
+                const int nb = min(32, T - w * 32);                 /* uniform */
 #pragma unroll 4
-                for (int b = 0; b < 32; ++b) {
-                    const int j = jb + b * 8;
-                    if (j < N_s) {
-                        const uint4 uj = fr[j];
-                        const float e0 = (float)(int)(uj.x - ui.x), e1 = (float)(int)(uj.y - ui.y), e2 = (float)(int)(uj.z - ui.z);
-                        const float r2 = e0 * (G0 * e0 + G1 * e1 + G2 * e2) + e1 * (G3 * e1 + G4 * e2) + G5 * e2 * e2;
-                        if (r2 < rb2 && j != ai) word |= 1u << b;
-                    }
+                for (int b = 0; b < nb; b += 2) {
+                    const uint4 ua = cj[b * 8], ub = cj[b * 8 + 8];
+                    const f32x2 E0 = pk2((float)(int)(ua.x - ui.x), (float)(int)(ub.x - ui.x));
+                    const f32x2 E1 = pk2((float)(int)(ua.y - ui.y), (float)(int)(ub.y - ui.y));
+                    const f32x2 E2 = pk2((float)(int)(ua.z - ui.z), (float)(int)(ub.z - ui.z));
+                    f32x2 A0 = mul2(G0, E0);
+                    A0 = fma2(G1, E1, A0);
+                    A0 = fma2(G2, E2, A0);
+                    f32x2 A1 = mul2(G3, E1);
+                    A1 = fma2(G4, E2, A1);
+                    f32x2 R = mul2(mul2(G5, E2), E2);
+                    R = fma2(E1, A1, R);
+                    R = fma2(E0, A0, R);
+                    float ra, rb;
+                    upk2(R, ra, rb);
+                    if (ra < rb2) word |= 1u << b;
+                    if (rb < rb2) word |= 2u << b;
                 }
+                /* candidates past the end of the system (padding) and the atom itself */
+                const int tmax = (N_s - l + 7) >> 3;                /* lane l owns t < tmax */
+                const int keep = tmax - w * 32;
+                if (keep < 32) word &= keep <= 0 ? 0u : ((1u << keep) - 1u);
+                if ((ai & 7) == l && (ai >> 8) == w) word &= ~(1u << ((ai >> 3) & 31));
+                if (!has) word = 0u;
             }
             mask[w] = word;
             mine += __popc(word);
         }
-        int c[8], NT = 0;
+        /* per-group populations of the four atoms of the task */
+        int NT = mine;
 #pragma unroll
-        for (int g = 0; g < 8; ++g) {
-            c[g] = __shfl_sync(0xffffffffu, mine, (lane & 24) | g);
-            NT += c[g];
-        }
+        for (int o = 1; o < 8; o <<= 1) NT += __shfl_xor_sync(0xffffffffu, NT, o);
         int niter = (NT + 15) >> 4;                                 /* u32 per lane: 16 entries per iteration */
         niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 8));
         niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16)); /* the four atoms of a task share the loop count */
@@ -420,28 +444,42 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
         }
         unsigned short *row = rows + (size_t)al * rc.pitch;
         if (fits) {
-            int m = 0;
+            /* lockstep over the rank m: entry (group g, rank m) goes to position a(m) + #{k < g : c_k > m},
+             * a(m) = sum_k min(c_k, m) -- the round-robin order over the bank groups */
+            int mmax = mine;
 #pragma unroll
-            for (int w = 0; w < 8; ++w) {
-                unsigned word = mask[w];
-                while (word) {
-                    const int b = __ffs(word) - 1;
-                    word &= word - 1u;
-                    const int j = w * 256 + b * 8 + l;
-                    const uint4 uj = fr[j];
-                    const int s0 = image_shift(uj.x, ui.x), s1 = image_shift(uj.y, ui.y), s2 = image_shift(uj.z, ui.z);
-                    unsigned slot = (unsigned)j;
-                    if ((s0 | s1 | s2) != 0) {
-                        const unsigned gd = gtab[j];
-                        const int act = (int)(gd >> 16) & 7, sg = (int)(gd >> 19) & 7;
-                        const int mm = (s0 != 0) | ((s1 != 0) << 1) | ((s2 != 0) << 2);
-                        const int want = (s0 > 0) | ((s1 > 0) << 1) | ((s2 > 0) << 2);
-                        if ((mm & ~act) != 0 || ((sg ^ want) & mm) != 0) misc->overflow = 1;   /* cannot happen: see ghost_table */
-                        slot = (gd & 0xffffu) + 8u * (unsigned)ghost_rank(mm, act);
+            for (int o = 1; o < 32; o <<= 1) mmax = max(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
+            unsigned cur = mask[0];
+            int wi = 0, a = 0;
+            const unsigned below = (1u << l) - 1u;
+            for (int m = 0; m < mmax; ++m) {
+                const bool pred = m < mine;
+                const unsigned bal = __ballot_sync(0xffffffffu, pred);
+                const unsigned byte = (bal >> (8 * q)) & 0xffu;
+                if (pred) {
+                    while (cur == 0u) {
+                        ++wi;
+                        cur = wi == 1 ? mask[1] : wi == 2 ? mask[2] : wi == 3 ? mask[3] : wi == 4 ? mask[4]
+                            : wi == 5 ? mask[5] : wi == 6 ? mask[6] : mask[7];
                     }
-                    row[row_index(rr_position(c, l, m))] = (unsigned short)(slot << 4);
-                    m += 1;
+                    const int b = __ffs(cur) - 1;
+                    cur &= cur - 1u;
+                    const int j = ((wi * 32 + b) << 3) + l;
+                    const uint4 uj = fr[j];
+                    const unsigned mm = wrap_bit(uj.x, ui.x) | (wrap_bit(uj.y, ui.y) << 1) | (wrap_bit(uj.z, ui.z) << 2);
+                    unsigned slot = (unsigned)j;
+                    if (mm) {
+                        const unsigned gd = gtab[j];
+                        const unsigned a0 = (gd >> 16) & 1u, a1 = (gd >> 17) & 1u;
+                        /* rank of the subset mm among the non-empty subsets of the active axes */
+                        const unsigned r = (mm & 1u) + (((mm >> 1) & 1u) << a0) + ((mm >> 2) << (a0 + a1)) - 1u;
+                        if ((mm & ~(gd >> 16)) & 7u) misc->overflow = 1;                  /* cannot happen: see ghost_table */
+                        slot = (gd & 0xffffu) + 8u * r;
+                    }
+                    const int p = a + __popc(byte & below);
+                    row[row_index(p)] = (unsigned short)(slot << 4);
                 }
+                a += __popc(byte);
             }
             /* padding: lane l owns the positions p = l mod 8 and pads them with the dummy of its bank group */
             for (int p = NT + ((l - NT) & 7); p < 16 * niter; p += 8) row[row_index(p)] = (unsigned short)((N8 + l) << 4);
@@ -542,7 +580,6 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         T x0 = 0, x1 = 0, x2 = 0, v0 = 0, v1 = 0, v2 = 0, f0 = 0, f1 = 0, f2 = 0, r0 = 0, r1 = 0, r2 = 0;
         T ws0 = 0, ws1 = 0, ws2 = 0, im = 0, mass = 0;
         int ty = 0;
-        unsigned gdesc = 0u;
         if (own) {
             const T *x = (const T *)d.pos + 3 * gi, *v = (const T *)d.vel + 3 * gi;
             x0 = x[0]; x1 = x[1]; x2 = x[2]; v0 = v[0]; v1 = v[1]; v2 = v[2];
@@ -555,6 +592,9 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const T hdt = (T)c.hdt, dt = (T)c.dt;
         cluster.sync();                               /* constants visible; previous system fully retired everywhere */
 
+#ifdef TS_RES_TIMING
+        long long prof_acc[12] = { 0 }, prof_t = clock64();
+#endif
         for (int n = 0; n <= n_steps; ++n) {
             const int nb = n & 1;
             if (n > 0) {
@@ -580,14 +620,18 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     T a = x0 - r0, b = x1 - r1, cc = x2 - r2;
                     moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
                 }
+                TICK(0);
                 cl_wait();                            /* every CTA of the cluster has finished reading the old positions */
+                TICK(1);
                 if (own) {
                     if (moved)
                         for (int r = 0; r < CL; ++r) cluster.map_shared_rank(misc, r)->flags[nb] = 1;
-                    publish_atom<T>(cluster, CL, posb, zt, ai, gdesc, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, true, true);
+                    publish_home<T>(cluster, CL, posb, zt, ai, x0 - ws0, x1 - ws1, x2 - ws2, ty);
                 }
+                TICK(2);
                 cl_arrive();
                 cl_wait();                            /* new positions (and the rebuild flag) visible everywhere */
+                TICK(3);
             }
             const bool rebuild = (n == 0) || (misc->flags[nb] != 0);
             if (rebuild) {
@@ -609,33 +653,40 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     r0 = x0; r1 = x1; r2 = x2;
                     const uint4 u = make_uint4(frac_to_u32(fa), frac_to_u32(fb), frac_to_u32(fc), 0u);
                     for (int r = 0; r < CL; ++r) cluster.map_shared_rank(fr, r)[ai] = u;
-                    publish_atom<T>(cluster, CL, posb, zt, ai, 0u, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, true, false);
+                    publish_home<T>(cluster, CL, posb, zt, ai, x0 - ws0, x1 - ws1, x2 - ws2, ty);
                 }
                 if (tid < 8) {                        /* the far-away dummy neighbours (list padding), one per bank group */
                     const T far = (T)1e15;
                     st_pos(posb, (unsigned)(N8 + tid) * 16u, zt, far, far, far, 0);
                 }
                 cluster.sync();                       /* fractions and home slots complete in every CTA */
+                TICK(4);
                 ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
-                if (own) {
-                    gdesc = misc->overflow ? 0u : gtab[ai];   /* on overflow (flagged) nothing is written past the slots */
-                    publish_atom<T>(cluster, CL, posb, zt, ai, gdesc, x0 - ws0, x1 - ws1, x2 - ws2, ty, gh, false, true);
-                }
-                cluster.sync();                       /* ghost slots complete in every CTA */
+                TICK(5);
+                TICK(6);
                 build_phase(rc, fr, gtab, rows, cnt, G, G[6], a_begin, A_own, N_s, N8, misc);
                 __syncthreads();
+                TICK(7);
             }
+            ghost_pass<T>(posb, zt, gtab, gh, N_s);              /* images of the new home positions, local */
+            __syncthreads();
+            TICK(10);
             const bool last = n == n_steps;
             if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
             else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
+            TICK(8);
             cl_arrive();                              /* this CTA no longer reads the positions of step n */
             __syncthreads();
+            TICK(9);
             if (own) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
                 if (n > 0) { v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im); }
             }
         }
         cl_wait();                                    /* pairs the last arrive */
+#ifdef TS_RES_TIMING
+        if (tid == 0) for (int k = 0; k < 12; ++k) atomicAdd(&g_res_prof[k], (unsigned long long)prof_acc[k]);
+#endif
         /* ---- store the system (R16): x, v at t + n dt, F(x), E, W, KE */
         double ke = 0.0;
         if (own) {
@@ -709,7 +760,7 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.CL = CL; c.A = A; c.pitch = pitch; c.NS = need_slots; c.nwarps = nwarps;
     unsigned o = 0;
     c.o_pos = o; o += up16((unsigned)(c.NS * 4 * w));
-    c.o_fr = o; o += up16((unsigned)nmax * 16u);
+    c.o_fr = o; o += up16((unsigned)(nmax + 16) * 16u);          /* padded: the builder tests two candidates per trip */
     c.o_gtab = o; o += up16((unsigned)nmax * 4u);
     c.o_rows = o; o += up16((unsigned)A * (unsigned)pitch * 2u);
     c.o_fs = o; o += up16((unsigned)(3 * A * w));
@@ -757,6 +808,7 @@ bool resident_supported(ts_state *st)
     }
     if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
     int ns = (((int)ceil(need_slots) + 7) / 8) * 8;
+    if (getenv("TS_RES_NS")) ns = atoi(getenv("TS_RES_NS"));
     if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
     if (ns < ((nmax + 7) & ~7) + 16) return false;
     double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
@@ -765,9 +817,11 @@ bool resident_supported(ts_state *st)
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     ResCfg best; bool have = false;
+    const char *force_cl = getenv("TS_RES_CL");
     for (int CL = 1; CL <= 8; CL *= 2) {
         ResCfg c;
         memset(&c, 0, sizeof c);
+        if (force_cl && atoi(force_cl) != CL) continue;
         if (!res_layout(c, CL, nmax, need_row, ns, d.dtype, d.n_types)) continue;
         best = c; have = true;
         if ((long long)S * CL >= (nsm * 3) / 4 || c.A <= 64) break;   /* enough CTAs to occupy the chip */
@@ -826,4 +880,18 @@ ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want
     st->last_engine = 1;
     st->list_built = false;          /* the general engine's list no longer matches the positions */
     return TS_OK;
+}
+
+/* debugging aid (only with -DTS_RES_TIMING): summed cycles per phase of warp 0 over all CTAs, then reset */
+extern "C" int ts_debug_resident_profile(unsigned long long *out16)
+{
+#ifdef TS_RES_TIMING
+    unsigned long long z[16] = { 0 };
+    if (cudaMemcpyFromSymbol(out16, g_res_prof, sizeof z) != cudaSuccess) return 1;
+    cudaMemcpyToSymbol(g_res_prof, z, sizeof z);
+    return 0;
+#else
+    (void)out16;
+    return 2;
+#endif
 }
