@@ -57,7 +57,7 @@ namespace cg = cooperative_groups;
 struct ResCfg {
     int CL;            /* CTAs per system = cluster size                       */
     int A;             /* atoms per CTA, capacity (multiple of 4)              */
-    int pitch;         /* u16 entries per list row, pitch mod 64 in {16, 48}   */
+    int pitch;         /* u16 entries per list row, a multiple of 32           */
     int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
@@ -118,11 +118,26 @@ template <typename T> __device__ __forceinline__ T t_floor(T x);
 template <> __device__ __forceinline__ float t_floor<float>(float x) { return floorf(x); }
 template <> __device__ __forceinline__ double t_floor<double>(double x) { return floor(x); }
 
-/* u16 index of list slot p (p = 8 k + lane) inside a row: pairs of k interleaved per lane */
-__device__ __forceinline__ int row_index(int p)
+/* u16 index of list slot p (p = 8 k + lane) inside a row: the four k of a trip are contiguous per lane */
+/* When the pitch is a multiple of 64 entries (rows 0 modulo 128 bytes apart) the odd rows store their
+ * trips pairwise swapped (sw = 1), so that the 64-bit row loads of the two quarter-warps that share a
+ * shared-memory phase never hit the same banks. */
+__device__ __forceinline__ int row_index(int p, int sw)
 {
     int k = p >> 3, l = p & 7;
-    return ((k >> 1) << 4) + (l << 1) + (k & 1);
+    return (((k >> 2) ^ sw) << 5) + (l << 2) + (k & 3);
+}
+
+/* Home slot of atom j.  The bank group of a slot is slot mod 8; atoms that follow each other in a
+ * regular pattern (a lattice written cell by cell) would load the groups of a neighbour list very
+ * unevenly, so every block of eight atoms is rotated by a hash of the block number.  The last block
+ * is not rotated: the unused slots stay the ones >= N_s.  Everything built from the positions (fr,
+ * gtab, the rows) lives in SLOT space; only the owner of an atom knows its index. */
+__device__ __forceinline__ int hslot(int j, int N8)
+{
+    const unsigned b = (unsigned)j >> 3;
+    const unsigned h = (int)b == (N8 >> 3) - 1 ? 0u : (b * 0x9E3779B1u) >> 29;
+    return (j & ~7) | (int)(((unsigned)j + h) & 7u);
 }
 
 /* ------------------------------------------------------------------ ghosts
@@ -222,18 +237,63 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
     return d;
 }
 
+/* ------------------------------------------------------------------ shared-space addressing */
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float4 lds128(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 lds64(unsigned a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+
+/* one packed step of the fp32 Lennard-Jones force loop: the two pairs (xi, pa) and (xi, pb) */
+__device__ __forceinline__ void lj_pair2(const float4 &pa, const float4 &pb, float xix, float xiy, float xiz, float rc2,
+                                         f32x2 C12, f32x2 C6, f32x2 &FX, f32x2 &FY, f32x2 &FZ)
+{
+    const f32x2 RX = pk2(pa.x - xix, pb.x - xix), RY = pk2(pa.y - xiy, pb.y - xiy), RZ = pk2(pa.z - xiz, pb.z - xiz);
+    f32x2 R2 = mul2(RX, RX);
+    R2 = fma2(RY, RY, R2);
+    R2 = fma2(RZ, RZ, R2);
+    float r2a, r2b;
+    upk2(R2, r2a, r2b);
+    float ia, ib;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
+    const float ma = r2a < rc2 ? 1.0f : 0.0f, mb = r2b < rc2 ? 1.0f : 0.0f;   /* strict (R9) */
+    const f32x2 I = mul2(pk2(ia, ib), pk2(ma, mb));
+    const f32x2 I2 = mul2(I, I);
+    const f32x2 I6 = mul2(I2, I);
+    const f32x2 P = fma2(I6, C12, C6);
+    const f32x2 G = mul2(mul2(I6, I), P);              /* g = V'(r)/r = ir2 ir6 (6 c1 - 12 c0 ir6) */
+    FX = fma2(G, RX, FX);
+    FY = fma2(G, RY, FY);
+    FZ = fma2(G, RZ, FZ);
+}
+
 /* Forces of the CTA's own atoms from the shared-memory list; E and W partials into red (fp64).
- * FAST = fp32 Lennard-Jones, one type, forces only: the two pairs of a lane share packed ops. */
+ * A row is read in TRIPS of 32 entries: lane l of the atom's quarter-warp loads its four entries of
+ * the trip with one 64-bit load (row_index).  FAST = fp32 Lennard-Jones, one type, forces only: the
+ * pairs of a lane share packed ops two by two. */
 template <typename T, int KIND, bool NT1, bool EV>
 __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char *posb, const unsigned short *rows,
                                            const unsigned *cnt, const PotEntry<T> *tab, T *fs, int a_begin, int A_own,
-                                           int NT, double *red)
+                                           int N8, int NT, double *red)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
     const unsigned zt = (unsigned)rc.NS * 16u;
     const int ntasks = (A_own + 3) >> 2;
     constexpr bool FAST = (sizeof(T) == 4) && KIND == TS_LJ && NT1 && !EV;
+    const unsigned pos_sa = smem_u32(posb);
+    const unsigned row_sa0 = smem_u32(rows) + (unsigned)q * (unsigned)rc.pitch * 2u + (unsigned)l * 8u;
+    const unsigned task_stride = 4u * (unsigned)rc.pitch * 2u;
+    const unsigned sw = (rc.pitch & 63) == 0 ? (unsigned)(q & 1) : 0u;
     double acc8[EV ? 7 : 1];
     if (EV)
 #pragma unroll
@@ -242,54 +302,45 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char
         T ev[7] = { 0, 0, 0, 0, 0, 0, 0 };
         const int al = task * 4 + q;
         const bool has = al < A_own;
-        const int ai = a_begin + (has ? al : 0);
-        const P3<T> xi = ld_pos(posb, (unsigned)ai * 16u, zt, (T)0);
-        const int niter = (int)cnt[task];                       /* the same for the four atoms of a task */
-        const unsigned *row = (const unsigned *)(rows + (size_t)al * rc.pitch) + l;
-        const PotEntry<T> pe1 = tab[NT1 ? 0 : xi.ty * NT];
-        const int tirow = xi.ty * NT;
+        const int ai = hslot(a_begin + (has ? al : 0), N8);     /* home slot of the atom */
+        const int ntrip = (int)cnt[task];                       /* the same for the four atoms of a task */
+        const unsigned ra = row_sa0 + (unsigned)task * task_stride;
         T fx = 0, fy = 0, fz = 0;
         if (FAST) {
-            const float xix = (float)xi.x, xiy = (float)xi.y, xiz = (float)xi.z, rc2 = (float)pe1.rc2;
+            const float4 xi4 = lds128(pos_sa + (unsigned)ai * 16u);
+            const PotEntry<T> pe1 = tab[0];
+            const float xix = xi4.x, xiy = xi4.y, xiz = xi4.z, rc2 = (float)pe1.rc2;
             const float m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
             const f32x2 C12 = pk2(m12, m12), C6 = pk2(p6, p6);
             f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
-#pragma unroll 2
-            for (int k = 0; k < niter; ++k) {
-                const unsigned e2 = row[k * 8];
-                const float4 pa = *(const float4 *)(posb + (e2 & 0xffffu));
-                const float4 pb = *(const float4 *)(posb + (e2 >> 16));
-                const f32x2 RX = pk2(pa.x - xix, pb.x - xix), RY = pk2(pa.y - xiy, pb.y - xiy), RZ = pk2(pa.z - xiz, pb.z - xiz);
-                f32x2 R2 = mul2(RX, RX);
-                R2 = fma2(RY, RY, R2);
-                R2 = fma2(RZ, RZ, R2);
-                float r2a, r2b;
-                upk2(R2, r2a, r2b);
-                float ia, ib;
-                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));
-                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
-                const float ma = r2a < rc2 ? 1.0f : 0.0f, mb = r2b < rc2 ? 1.0f : 0.0f;   /* strict (R9) */
-                const f32x2 I = mul2(pk2(ia, ib), pk2(ma, mb));
-                const f32x2 I2 = mul2(I, I);
-                const f32x2 I6 = mul2(I2, I);
-                const f32x2 P = fma2(I6, C12, C6);
-                const f32x2 G = mul2(mul2(I6, I), P);              /* g = V'(r)/r = ir2 ir6 (6 c1 - 12 c0 ir6) */
-                FX = fma2(G, RX, FX);
-                FY = fma2(G, RY, FY);
-                FZ = fma2(G, RZ, FZ);
+            uint2 e = lds64(ra + (sw << 6));
+            for (int t = 0; t < ntrip; ++t) {
+                const float4 p0 = lds128(pos_sa + (e.x & 0xffffu));
+                const float4 p1 = lds128(pos_sa + (e.x >> 16));
+                const float4 p2 = lds128(pos_sa + (e.y & 0xffffu));
+                const float4 p3 = lds128(pos_sa + (e.y >> 16));
+                e = lds64(ra + (((unsigned)(t + 1) ^ sw) << 6));      /* next trip's entries (one past the end is still inside smem) */
+                lj_pair2(p0, p1, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
+                lj_pair2(p2, p3, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
             }
             float a, b;
             upk2(FX, a, b); fx = (T)(a + b);
             upk2(FY, a, b); fy = (T)(a + b);
             upk2(FZ, a, b); fz = (T)(a + b);
         } else {
-#pragma unroll 2
-            for (int k = 0; k < niter; ++k) {
-                const unsigned e2 = row[k * 8];
-                const P3<T> x0 = ld_pos(posb, e2 & 0xffffu, zt, (T)0);
-                const P3<T> x1 = ld_pos(posb, e2 >> 16, zt, (T)0);
+            const P3<T> xi = ld_pos(posb, (unsigned)ai * 16u, zt, (T)0);
+            const PotEntry<T> pe1 = tab[NT1 ? 0 : xi.ty * NT];
+            const int tirow = xi.ty * NT;
+            for (int t = 0; t < ntrip; ++t) {
+                const uint2 e = lds64(ra + (((unsigned)t ^ sw) << 6));
+                const P3<T> x0 = ld_pos(posb, e.x & 0xffffu, zt, (T)0);
+                const P3<T> x1 = ld_pos(posb, e.x >> 16, zt, (T)0);
+                const P3<T> x2 = ld_pos(posb, e.y & 0xffffu, zt, (T)0);
+                const P3<T> x3 = ld_pos(posb, e.y >> 16, zt, (T)0);
                 pair_accum<T, KIND, NT1, EV>(xi, x0, pe1, tab, tirow, fx, fy, fz, ev);
                 pair_accum<T, KIND, NT1, EV>(xi, x1, pe1, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x2, pe1, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x3, pe1, tab, tirow, fx, fy, fz, ev);
             }
         }
 #pragma unroll
@@ -391,7 +442,7 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
     for (int task = warp; task < ntasks; task += rc.nwarps) {
         const int al = task * 4 + q;
         const bool has = al < A_own;
-        const int ai = a_begin + (has ? al : 0);
+        const int ai = hslot(a_begin + (has ? al : 0), N8);     /* slot of the atom: the build works in slot space */
         const uint4 ui = fr[ai];
         unsigned mask[8];
         int mine = 0;
@@ -430,41 +481,54 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
             mask[w] = word;
             mine += __popc(word);
         }
-        /* per-group populations of the four atoms of the task */
-        int NT = mine;
+        /* entries of the lanes below (exclusive prefix inside the quarter-warp) and of the whole atom */
+        int inc = mine;
 #pragma unroll
-        for (int o = 1; o < 8; o <<= 1) NT += __shfl_xor_sync(0xffffffffu, NT, o);
-        int niter = (NT + 15) >> 4;                                 /* u32 per lane: 16 entries per iteration */
+        for (int o = 1; o < 8; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, inc, o, 8);
+            if (l >= o) inc += v;
+        }
+        const int NT = __shfl_sync(0xffffffffu, inc, 7, 8);
+        int cq[8];                                                    /* populations of the eight bank groups of the atom */
+#pragma unroll
+        for (int c = 0; c < 8; ++c) cq[c] = __shfl_sync(0xffffffffu, mine, c, 8);
+        int niter = (NT + 31) >> 5;                                 /* trips: u64 per lane, 32 entries per trip */
         niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 8));
         niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16)); /* the four atoms of a task share the loop count */
-        const bool fits = 16 * niter <= rc.pitch && !ovf;
+        const bool fits = 32 * niter <= rc.pitch && !ovf;
         if (!fits) {
             if (lane == 0) misc->overflow = 1;
             niter = 0;
         }
         unsigned short *row = rows + (size_t)al * rc.pitch;
-        if (fits) {
-            /* lockstep over the rank m: entry (group g, rank m) goes to position a(m) + #{k < g : c_k > m},
-             * a(m) = sum_k min(c_k, m) -- the round-robin order over the bank groups */
-            int mmax = mine;
+        const int sw = (rc.pitch & 63) == 0 ? (q & 1) : 0;
+        if (fits && niter > 0) {
+            /* Placement.  The pair loop reads R = 4 niter rows of eight entries; entry (row, column) is read by
+             * lane `column`, and one shared-memory wavefront serves a row when its eight bank groups differ.
+             * Lane l holds the hits of bank group l: its first R hits fill column l from the top (column = bank
+             * group, so those never collide), the rest of the column is padded with the far-away dummy of group
+             * l.  A group with more than R hits overflows: those hits take the free cells of the other columns in
+             * column-major order, where they collide with their own group's column once each -- the minimum. */
+            const int R = 4 * niter;
+            const int o_l = max(0, mine - R), f_l = max(0, R - mine);
+            int io = o_l, jf = f_l;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) mmax = max(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
-            unsigned cur = mask[0];
-            int wi = 0, a = 0;
-            const unsigned below = (1u << l) - 1u;
-            for (int m = 0; m < mmax; ++m) {
-                const bool pred = m < mine;
-                const unsigned bal = __ballot_sync(0xffffffffu, pred);
-                const unsigned byte = (bal >> (8 * q)) & 0xffu;
-                if (pred) {
-                    while (cur == 0u) {
-                        ++wi;
-                        cur = wi == 1 ? mask[1] : wi == 2 ? mask[2] : wi == 3 ? mask[3] : wi == 4 ? mask[4]
-                            : wi == 5 ? mask[5] : wi == 6 ? mask[6] : mask[7];
-                    }
-                    const int b = __ffs(cur) - 1;
-                    cur &= cur - 1u;
-                    const int j = ((wi * 32 + b) << 3) + l;
+            for (int o = 1; o < 8; o <<= 1) {
+                const int vo = __shfl_up_sync(0xffffffffu, io, o, 8), vf = __shfl_up_sync(0xffffffffu, jf, o, 8);
+                if (l >= o) { io += vo; jf += vf; }
+            }
+            const int O = __shfl_sync(0xffffffffu, io, 7, 8);             /* overflow entries of the atom */
+            const int F_l = jf - f_l;                                     /* free cells in the columns below l */
+            const int recv = min(max(O - F_l, 0), f_l);                   /* overflow entries that land in column l */
+            int u = io - o_l;                                             /* number of my first overflow entry */
+            int m = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) {
+                unsigned word = mask[w];
+                while (word) {
+                    const int b = __ffs(word) - 1;
+                    word &= word - 1u;
+                    const int j = ((w * 32 + b) << 3) + l;
                     const uint4 uj = fr[j];
                     const unsigned mm = wrap_bit(uj.x, ui.x) | (wrap_bit(uj.y, ui.y) << 1) | (wrap_bit(uj.z, ui.z) << 2);
                     unsigned slot = (unsigned)j;
@@ -476,13 +540,27 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
                         if ((mm & ~(gd >> 16)) & 7u) misc->overflow = 1;                  /* cannot happen: see ghost_table */
                         slot = (gd & 0xffffu) + 8u * r;
                     }
-                    const int p = a + __popc(byte & below);
-                    row[row_index(p)] = (unsigned short)(slot << 4);
+                    int prow = m, pcol = l;
+                    if (m >= R) {                                          /* the u-th free cell, column-major */
+                        int P = 0, Fc = 0;
+                        pcol = 0;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) {                      /* columns whose free cells all come before cell u */
+                            P += R - min(R, cq[c]);
+                            if (P <= u) { pcol = c + 1; Fc = P; }
+                        }
+                        int cc = 0;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) cc = pcol == c ? cq[c] : cc;
+                        prow = cc + (u - Fc);
+                        ++u;
+                    }
+                    row[row_index(8 * prow + pcol, sw)] = (unsigned short)(slot << 4);
+                    ++m;
                 }
-                a += __popc(byte);
             }
-            /* padding: lane l owns the positions p = l mod 8 and pads them with the dummy of its bank group */
-            for (int p = NT + ((l - NT) & 7); p < 16 * niter; p += 8) row[row_index(p)] = (unsigned short)((N8 + l) << 4);
+            /* padding of my column below my own hits and the overflow entries it received */
+            for (int r = min(mine, R) + recv; r < R; ++r) row[row_index(8 * r + l, sw)] = (unsigned short)((N8 + l) << 4);
         }
         if (lane == 0) cnt[task] = (unsigned)niter;
         if (has && l == 0) nnz += (unsigned)NT;
@@ -576,6 +654,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         /* ---- owner state */
         const bool own = tid < A_own;
         const int ai = a_begin + tid;                 /* system-local atom index  */
+        const int hs = hslot(ai, N8);                 /* its home slot            */
         const long long gi = (long long)g0 + ai;      /* global atom index        */
         T x0 = 0, x1 = 0, x2 = 0, v0 = 0, v1 = 0, v2 = 0, f0 = 0, f1 = 0, f2 = 0, r0 = 0, r1 = 0, r2 = 0;
         T ws0 = 0, ws1 = 0, ws2 = 0, im = 0, mass = 0;
@@ -626,7 +705,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 if (own) {
                     if (moved)
                         for (int r = 0; r < CL; ++r) cluster.map_shared_rank(misc, r)->flags[nb] = 1;
-                    publish_home<T>(cluster, CL, posb, zt, ai, x0 - ws0, x1 - ws1, x2 - ws2, ty);
+                    publish_home<T>(cluster, CL, posb, zt, hs, x0 - ws0, x1 - ws1, x2 - ws2, ty);
                 }
                 TICK(2);
                 cl_arrive();
@@ -652,8 +731,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     ws2 = wa * gh[2] + wb * gh[5] + wc * gh[8];
                     r0 = x0; r1 = x1; r2 = x2;
                     const uint4 u = make_uint4(frac_to_u32(fa), frac_to_u32(fb), frac_to_u32(fc), 0u);
-                    for (int r = 0; r < CL; ++r) cluster.map_shared_rank(fr, r)[ai] = u;
-                    publish_home<T>(cluster, CL, posb, zt, ai, x0 - ws0, x1 - ws1, x2 - ws2, ty);
+                    for (int r = 0; r < CL; ++r) cluster.map_shared_rank(fr, r)[hs] = u;
+                    publish_home<T>(cluster, CL, posb, zt, hs, x0 - ws0, x1 - ws1, x2 - ws2, ty);
                 }
                 if (tid < 8) {                        /* the far-away dummy neighbours (list padding), one per bank group */
                     const T far = (T)1e15;
@@ -672,8 +751,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             __syncthreads();
             TICK(10);
             const bool last = n == n_steps;
-            if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
-            else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, NT, red);
+            if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
+            else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
             TICK(8);
             cl_arrive();                              /* this CTA no longer reads the positions of step n */
             __syncthreads();
@@ -750,8 +829,7 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     int A = ((((nmax + CL - 1) / CL) + 3) / 4) * 4;
     const int max_threads = dtype == TS_F32 ? RES_MAX_THREADS : RES_MAX_THREADS_F64;
     if (A > max_threads) return false;
-    int pitch = 32 * ((need_row - 16 + 31) / 32) + 16;           /* multiple of 16, rows 32 bytes apart modulo 128 */
-    if (pitch < 48) pitch = 48;
+    int pitch = 32 * ((need_row + 31) / 32);                     /* whole trips of 32 entries */
     int ntasks = A / 4, maxw = max_threads / 32;
     int passes = (ntasks + maxw - 1) / maxw;
     int nwarps = (ntasks + passes - 1) / passes;
@@ -812,7 +890,7 @@ bool resident_supported(ts_state *st)
     if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
     if (ns < ((nmax + 7) & ~7) + 16) return false;
     double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
-    int need_row = (int)ceil(need * slack) + 16;                   /* + padding to 16 */
+    int need_row = (int)ceil(need * slack);
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);

@@ -31,15 +31,18 @@ __device__ __forceinline__ void normals3(const unsigned w[4], double xi[3])
     sincospi(2.0 * u3, &sn2, &cs2);
     xi[0] = r0 * cs; xi[1] = r0 * sn; xi[2] = r1 * cs2;
 }
+/* fp32 runs (R19: log / sin / cos may be evaluated in fp32): the hardware approximations (MUFU.LG2, MUFU.SQRT,
+ * MUFU.SIN / COS on an argument reduced to [-pi, pi)) -- absolute error ~1e-6 on a unit normal, far below the fp32
+ * rounding of the velocity update it feeds; no trajectory parity is asked of fp32 runs. */
 __device__ __forceinline__ void normals3(const unsigned w[4], float xi[3])
 {
     const float s = 2.3283064365386963e-10f;
-    float u0 = ((float)w[0] + 0.5f) * s, u1 = ((float)w[1] + 0.5f) * s;
-    float u2 = ((float)w[2] + 0.5f) * s, u3 = ((float)w[3] + 0.5f) * s;
-    float r0 = sqrtf(-2.0f * logf(u0)), r1 = sqrtf(-2.0f * logf(u2));
-    float sn, cs, sn2, cs2;
-    sincospif(2.0f * u1, &sn, &cs);
-    sincospif(2.0f * u3, &sn2, &cs2);
-    xi[0] = r0 * cs; xi[1] = r0 * sn; xi[2] = r1 * cs2;
+    const float u0 = ((float)w[0] + 0.5f) * s, u1 = ((float)w[1] + 0.5f) * s;
+    const float u2 = ((float)w[2] + 0.5f) * s, u3 = ((float)w[3] + 0.5f) * s;
+    float r0, r1;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(-1.3862943611198906f * __log2f(u0)));   /* -2 ln u = -2 ln2 lg2 u */
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r1) : "f"(-1.3862943611198906f * __log2f(u2)));
+    const float t1 = fmaf(6.283185307179586f, u1, -3.141592653589793f);                      /* cos(t + pi) = -cos t */
+    const float t3 = fmaf(6.283185307179586f, u3, -3.141592653589793f);
+    xi[0] = -r0 * __cosf(t1); xi[1] = -r0 * __sinf(t1); xi[2] = -r1 * __cosf(t3);
 }
-

@@ -182,3 +182,22 @@ def test_fp32_replay_parity_after_md(ts, orc, engine):
     scale = np.maximum(np.abs(o["E"]), o["Eabs"])
     assert np.all(np.abs(st.numpy("energy") - o["E"]) <= 2e-5 * scale)
     st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_fp32_baoab_noise_follows_the_oracle_stream(ts, orc, engine):
+    """fp32 runs evaluate log / sin / cos with the hardware approximations (R19).  After ONE BAOAB
+    step the fp32 velocities must still be the oracle's to fp32 accuracy: same Philox counters, same
+    Box-Muller pairing of the words, same signs.  The kick from the noise is c2 sqrt(kT/m) xi
+    (~2.5e-4 A/fs per unit normal), so 2e-7 A/fs absolute resolves a 1e-3 error on xi."""
+    b = wl.cfg2(n_systems=2, dtype="f32")
+    md = dict(b.md)
+    o = orc.md_run(b, "baoab", md["dt"], 1, temperature=md["temperature"], friction=md["friction"],
+                   seed=md["seed"], sys_uid=b.sys_uid)
+    st = ts.SimState(b, engine=engine)
+    st.md_step(md, 1)
+    assert st.poll().flags == 0
+    dv = np.abs(st.numpy("vel").astype(np.float64) - o["vel"])
+    assert dv.max() <= 2e-7
+    assert np.abs(st.numpy("pos").astype(np.float64) - o["pos"]).max() <= 2e-5
+    st.close()
