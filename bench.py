@@ -168,7 +168,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--md-steps", type=int, default=100, help="MD steps per ts_md_step call (= per bench step)")
+    ap.add_argument("--md-steps", type=int, default=1000,
+                    help="MD steps per ts_md_step call (= per bench step); BASELINE.json configs[1] runs 1000 steps")
     ap.add_argument("--systems", type=int, default=64)
     ap.add_argument("--engine", type=int, default=1)
     ap.add_argument("--impl", default="ours")

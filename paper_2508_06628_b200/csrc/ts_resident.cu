@@ -83,6 +83,9 @@ __device__ unsigned long long g_res_prof[16];
 #endif
 
 __device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+/* "this CTA has finished READING the positions of the step": nothing was written, so no release fence is needed
+ * (the loads completed before their values were consumed); the matching wait still acquires */
+__device__ __forceinline__ void cl_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 /* ------------------------------------------------------------------ position slots */
@@ -754,7 +757,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
             else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
             TICK(8);
-            cl_arrive();                              /* this CTA no longer reads the positions of step n */
+            cl_arrive_relaxed();                      /* this CTA no longer reads the positions of step n */
             __syncthreads();
             TICK(9);
             if (own) {
