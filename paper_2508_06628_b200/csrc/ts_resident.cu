@@ -51,7 +51,7 @@ namespace cg = cooperative_groups;
 #define RES_MAX_THREADS 896         /* fp32; the fp64 kernels need twice the registers: 512 */
 #define RES_MAX_THREADS_F64 512
 #define RES_MAX_ATOMS 2047          /* builder hit masks cover 8 x 256 candidates */
-#define RES_MAX_SLOTS 4095          /* 16-bit byte offsets of 16-byte slots */
+#define RES_MAX_SLOTS 16376         /* list entries are 16-bit slot numbers; shared memory is the real limit */
 #define RES_SMEM_LIMIT (227 * 1024)
 
 struct ResCfg {
@@ -318,10 +318,10 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char
             f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
             uint2 e = lds64(ra + (sw << 6));
             for (int t = 0; t < ntrip; ++t) {
-                const float4 p0 = lds128(pos_sa + (e.x & 0xffffu));
-                const float4 p1 = lds128(pos_sa + (e.x >> 16));
-                const float4 p2 = lds128(pos_sa + (e.y & 0xffffu));
-                const float4 p3 = lds128(pos_sa + (e.y >> 16));
+                const float4 p0 = lds128(pos_sa + ((e.x & 0xffffu) << 4));
+                const float4 p1 = lds128(pos_sa + ((e.x >> 16) << 4));
+                const float4 p2 = lds128(pos_sa + ((e.y & 0xffffu) << 4));
+                const float4 p3 = lds128(pos_sa + ((e.y >> 16) << 4));
                 e = lds64(ra + (((unsigned)(t + 1) ^ sw) << 6));      /* next trip's entries (one past the end is still inside smem) */
                 lj_pair2(p0, p1, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
                 lj_pair2(p2, p3, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
@@ -336,10 +336,10 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char
             const int tirow = xi.ty * NT;
             for (int t = 0; t < ntrip; ++t) {
                 const uint2 e = lds64(ra + (((unsigned)t ^ sw) << 6));
-                const P3<T> x0 = ld_pos(posb, e.x & 0xffffu, zt, (T)0);
-                const P3<T> x1 = ld_pos(posb, e.x >> 16, zt, (T)0);
-                const P3<T> x2 = ld_pos(posb, e.y & 0xffffu, zt, (T)0);
-                const P3<T> x3 = ld_pos(posb, e.y >> 16, zt, (T)0);
+                const P3<T> x0 = ld_pos(posb, (e.x & 0xffffu) << 4, zt, (T)0);
+                const P3<T> x1 = ld_pos(posb, (e.x >> 16) << 4, zt, (T)0);
+                const P3<T> x2 = ld_pos(posb, (e.y & 0xffffu) << 4, zt, (T)0);
+                const P3<T> x3 = ld_pos(posb, (e.y >> 16) << 4, zt, (T)0);
                 pair_accum<T, KIND, NT1, EV>(xi, x0, pe1, tab, tirow, fx, fy, fz, ev);
                 pair_accum<T, KIND, NT1, EV>(xi, x1, pe1, tab, tirow, fx, fy, fz, ev);
                 pair_accum<T, KIND, NT1, EV>(xi, x2, pe1, tab, tirow, fx, fy, fz, ev);
@@ -558,12 +558,12 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
                         prow = cc + (u - Fc);
                         ++u;
                     }
-                    row[row_index(8 * prow + pcol, sw)] = (unsigned short)(slot << 4);
+                    row[row_index(8 * prow + pcol, sw)] = (unsigned short)slot;
                     ++m;
                 }
             }
             /* padding of my column below my own hits and the overflow entries it received */
-            for (int r = min(mine, R) + recv; r < R; ++r) row[row_index(8 * r + l, sw)] = (unsigned short)((N8 + l) << 4);
+            for (int r = min(mine, R) + recv; r < R; ++r) row[row_index(8 * r + l, sw)] = (unsigned short)(N8 + l);
         }
         if (lane == 0) cnt[task] = (unsigned)niter;
         if (has && l == 0) nnz += (unsigned)NT;
@@ -876,16 +876,21 @@ bool resident_supported(ts_state *st)
         for (int a = 0; a < 3; ++a)
             lmax = fmax(lmax, sqrt(g.h[3 * a] * g.h[3 * a] + g.h[3 * a + 1] * g.h[3 * a + 1] + g.h[3 * a + 2] * g.h[3 * a + 2]));
         double rb = d.r_list + 4.0 * eps_rel * lmax;
-        double images = 1.0;
+        double images = 1.0, images2 = 1.0;                       /* E[c + 1], E[(c + 1)^2] of the image count c of an atom */
         for (int k = 0; k < 3; ++k) {
             if (!(g.hperp[k] >= 2.0 * rb)) return false;          /* more than one image within r_list possible */
-            images *= 1.0 + fmin(1.0, 2.0 * rb / g.hperp[k]);
+            const double pk = fmin(1.0, 2.0 * rb / g.hperp[k]);   /* an atom is within rb of a face of axis k */
+            images *= 1.0 + pk;
+            images2 *= 1.0 + 3.0 * pk;
         }
         double nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
         need = fmax(need, nbar);
-        /* atoms + dummies + expected ghosts (uniform density) with 25 % head room; 8 more per bank group for the
-         * uneven fill of the eight per-group slot sequences */
-        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 1.25 * (images - 1.0) * n + 8.0 * 16.0);
+        /* atoms + dummies + ghosts.  The ghosts of a bank group occupy one of eight interleaved slot sequences, so the
+         * array needs 8 x the fullest group: mean + 4 sigma of a sum of n / 8 independent image counts (a lattice
+         * written cell by cell deviates systematically by ~2.5 sigma: measured on configs[1]), + 8 per group. */
+        const double mean_c = images - 1.0, var_c = fmax(0.0, (images2 - 2.0 * images + 1.0) - mean_c * mean_c);
+        const double per_group = mean_c * n / 8.0 + 4.0 * sqrt(var_c * n / 8.0) + 8.0;
+        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 8.0 * ceil(per_group));
     }
     if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
     int ns = (((int)ceil(need_slots) + 7) / 8) * 8;

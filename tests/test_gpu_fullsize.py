@@ -1,0 +1,164 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default engine selection,
+default slack): the oracle cannot run a whole batch in seconds, so each test checks (a) sampled systems element by
+element against the oracle (systems are independent, so the oracle evaluates a sampled system alone -- O7), and (b)
+properties that hold at any size (zero net force per system, no error flag, every stream id processed once).
+Tolerances are BASELINE.json:north_star's (see test_gpu_parity.py)."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ts():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2508_06628_b200 as m
+    m.lib()
+    return m
+
+
+def _sys_slice(b, s):
+    return slice(int(b.sys_offset[s]), int(b.sys_offset[s + 1]))
+
+
+def _replay_check(ts, orc, b, st, samples, fp32=True, e_tol=2e-5):
+    """R29 on sampled systems: the GPU's own positions go to the oracle; forces within 1e-4 max|F| (fp32) except
+    atoms in a pair within 1e-5 of r_c (counted); energies within e_tol of max(|E|, sum 1/2 |V|)."""
+    pos = st.numpy("pos").astype(np.float64)
+    F = st.numpy("force").astype(np.float64)
+    E = st.numpy("energy")
+    rc = b.potential.rc_max
+    for s in samples:
+        sl = _sys_slice(b, s)
+        one = wl.with_(wl.take(b, [s]), pos=pos[sl].copy())
+        o = orc.energy_forces(one)
+        i, j, S, r2 = orc.pairs(one.pos, one.cell[0], rc * (1.0 + 1e-4))
+        near = np.abs(np.sqrt(r2) - rc) < 1e-5 * max(1.0, rc / 8.5)
+        ok = np.ones(one.n_atoms, bool)
+        ok[i[near]] = False
+        assert (~ok).mean() < 0.02
+        fmax = np.linalg.norm(o["F"], axis=1).max()
+        tol = (1e-4 if fp32 else 1e-9) * fmax
+        assert np.abs(F[sl] - o["F"])[ok].max() <= tol, (s, np.abs(F[sl] - o["F"])[ok].max(), tol)
+        scale = max(abs(o["E"][0]), o["Eabs"][0])
+        assert abs(E[s] - o["E"][0]) <= e_tol * scale, (s, E[s], o["E"][0])
+
+
+def _net_force_is_zero(b, st, rel=2e-4):
+    F = st.numpy("force").astype(np.float64)
+    seg = np.add.reduceat(F, b.sys_offset[:-1].astype(np.int64), axis=0)
+    absseg = np.add.reduceat(np.abs(F), b.sys_offset[:-1].astype(np.int64), axis=0)
+    assert np.all(np.abs(seg) <= rel * absseg + 1e-12)
+
+
+def test_cfg2_full_fp32_as_benched(ts, orc):
+    """configs[1] exactly as bench.py launches it: 64 x 864, fp32, resident engine, BAOAB."""
+    b = wl.cfg2(n_systems=64, dtype="f32")
+    st = ts.SimState(b)
+    st.md_step(dict(b.md), 300)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 1 and rep.resident_rebuilds >= 64
+    assert np.array_equal(st.get_system_steps(), np.full(64, 300, np.uint64))
+    _replay_check(ts, orc, b, st, samples=(0, 31, 63))
+    _net_force_is_zero(b, st)
+    T = 2.0 * st.numpy("kinetic") / (3 * 864 * b.kB)
+    assert np.all((T > 40.0) & (T < 120.0))                  # thermostat at 80 K acts on every system
+    st.close()
+
+
+def test_cfg2_full_fp64_trajectory_of_sampled_systems(ts, orc):
+    """configs[1] fp64: positions of sampled systems after 100 BAOAB steps against the oracle run of that system
+    alone (the noise follows the system's uid, R18)."""
+    b = wl.cfg2(n_systems=64, dtype="f64")
+    md = dict(b.md)
+    st = ts.SimState(b)
+    st.md_step(md, 100)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 1
+    pos = st.numpy("pos")
+    for s in (5, 40):
+        one = wl.take(b, [s])
+        o = orc.md_run(one, "baoab", md["dt"], 100, temperature=md["temperature"], friction=md["friction"],
+                       seed=md["seed"], sys_uid=one.sys_uid)
+        assert np.abs(pos[_sys_slice(b, s)] - o["pos"]).max() <= 1e-8
+        assert abs(st.numpy("energy")[s] - o["E"][0]) <= 1e-9 * abs(o["E"][0])
+    st.close()
+
+
+def test_cfg3_full_ragged_morse_fp32(ts, orc):
+    """configs[2]: 512 ragged triclinic Cu systems (32..2048 atoms), Morse, E / F / W, then NVE steps."""
+    b = wl.cfg3(n_systems=512, dtype="f32")
+    n = np.diff(b.sys_offset)
+    samples = sorted({int(np.argmin(n)), int(np.argmax(n)), 7, 200, 511})
+    st = ts.SimState(b)
+    st.compute_forces(ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.nnz <= rep.nnz_capacity
+    F = st.numpy("force").astype(np.float64)
+    for s in samples:
+        sl = _sys_slice(b, s)
+        o = orc.energy_forces(wl.take(b, [s]))
+        fmax = np.linalg.norm(o["F"], axis=1).max()
+        assert np.abs(F[sl] - o["F"]).max() <= 1e-4 * fmax
+        scale = max(abs(o["E"][0]), o["Eabs"][0])
+        assert abs(st.numpy("energy")[s] - o["E"][0]) <= 1e-5 * scale
+        assert np.abs(st.numpy("virial")[s] - o["W"][0]).max() <= 1e-4 * (np.abs(o["W"][0]).max() + o["Eabs"][0])
+    _net_force_is_zero(b, st)
+    st.md_step(dict(b.md), 50)
+    assert st.poll().flags == 0
+    _replay_check(ts, orc, b, st, samples)
+    _net_force_is_zero(b, st)
+    st.close()
+
+
+def test_cfg4_full_slots_inflight_fire(ts, orc):
+    """configs[3] at its full slot count: 1024 slots x 256 atoms, FIRE with in-flight swaps (R22, R24, R30).  The
+    stream is cut at 1536 ids (the 4096-id run only repeats the same loop; bench-size slots are what matters here)."""
+    from paper_2508_06628_b200 import scheduler as sch
+    n_total = 1536
+    make = lambda ids: wl.cfg4(ids)
+    fire = dict(make([0]).fire, f_max=1e-4, max_steps=50000)
+    r = sch.InFlightRelaxer(make, n_total, fire, n_slots=1024, k_check=10)
+    res = r.run()
+    assert sorted(res) == list(range(n_total)) and r.unfinished == []
+    assert r.peak_resident <= 1024
+    n_conv = sum(1 for rec in res.values() if rec["status"] == ts.TS_FIRE_CONVERGED)
+    assert n_conv >= 0.95 * n_total                          # failed (max_steps) systems are reported, not counted
+    for sid in (0, 1023, 1024, 1535):
+        rec = res[sid]
+        if rec["status"] != ts.TS_FIRE_CONVERGED:
+            continue
+        o = orc.energy_forces(wl.with_(make([sid]), pos=rec["pos"]))
+        assert np.sqrt((o["F"] ** 2).sum(1)).max() < fire["f_max"]             # R30(ii)
+        assert abs(rec["energy"] - o["E"][0]) <= 1e-12 * max(abs(o["E"][0]), o["Eabs"][0])
+
+
+def test_cfg5_liquid_fp32_large_batch(ts, orc):
+    """configs[4] (R33): LJ liquid, 1000 atoms per system, pre-relaxed by the library's own soft-sphere FIRE, then NVE.
+    2048 systems (2 M atoms) here; bench-size 10^4 systems only scale the same launch.  Parity is on the first systems
+    (parity is unpinned at full size: DESIGN.md section 3) plus size-independent properties."""
+    S = 2048
+    start = wl.cfg5_start(range(S))
+    sf = ts.SimState(start)
+    sf.fire_step(dict(start.fire, f_max=1e-12, max_steps=10**6), 200)
+    assert sf.poll().flags == 0
+    relaxed = wl.with_(start, pos=sf.numpy("pos").astype(np.float64))
+    sf.close()
+    b = wl.cfg5_md(relaxed)
+    st = ts.SimState(b)
+    st.compute_forces(ts.TS_WANT_ENERGY)
+    assert st.poll().flags == 0
+    E0 = st.numpy("energy") + st.numpy("kinetic")
+    _replay_check(ts, orc, b, st, samples=(0, 1, S - 1), e_tol=1e-5)
+    st.md_step(dict(b.md), 200)
+    rep = st.poll()
+    assert rep.flags == 0
+    _replay_check(ts, orc, b, st, samples=(0, 1, S - 1))
+    _net_force_is_zero(b, st)
+    E1 = st.numpy("energy") + st.numpy("kinetic")
+    assert np.abs(E1 - E0).max() <= 5e-3 * 1000              # NVE drift per system over 200 steps, reduced units
+    st.close()
