@@ -194,61 +194,69 @@ __global__ void k_scatter(DevState d)
 
 __device__ __forceinline__ int floordiv(int a, int n) { int q = a / n; return (a % n < 0) ? q - 1 : q; }
 
-/* One warp per sorted slot p.  Lanes stride over the atoms of each stencil cell. */
+/* One quarter-warp (8 lanes) per sorted slot p, four consecutive slots per warp: sorted slots that follow each other
+ * sit in the same or in adjacent bins, so the four stencil walks of a warp stay converged and share their loads.  The
+ * lanes of a quarter stride over the atoms of each stencil bin; hits are compacted with a quarter-wide ballot.  The
+ * grid is capped (grid-stride over the slots): when no rebuild is due the launch costs a few microseconds. */
 template <int FILL>
-__global__ void k_nbr(DevState d)
+__global__ void __launch_bounds__(256) k_nbr(DevState d)
 {
     if (!d.status->need_rebuild) return;
-    long long p = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
-    int lane = threadIdx.x & 31;
-    if (p >= d.N) return;
-    int s = d.sysidx[p];                 /* sorted slots of a system occupy the system's own range */
-    if (FILL && d.nbr_len[s] < 0) return;
-    const SysGeom &g = d.geom[s];
-    int a0 = d.sysoff[s];
-    int base = a0 + s;
-    double4 me = d.spos[p];
-    int li = (int)__double_as_longlong(me.w);
-    int lin = d.atom_cell[a0 + li] - base;
-    int nb0 = g.nb[0], nb1 = g.nb[1], nb2 = g.nb[2];
-    int c2 = lin % nb2, c1 = (lin / nb2) % nb1, c0 = lin / (nb2 * nb1);
-    int D0 = g.D[0], D1 = g.D[1], D2 = g.D[2];
-    double R2 = d.r_list2;
-    int cnt = 0;
-    long long off = FILL ? d.nbr_off[a0 + li] : 0;
-    unsigned lt = (1u << lane) - 1u;
-    for (int e0 = c0 - D0; e0 <= c0 + D0; ++e0) {
-        int s0 = floordiv(e0, nb0), b0 = e0 - s0 * nb0;
-        for (int e1 = c1 - D1; e1 <= c1 + D1; ++e1) {
-            int s1 = floordiv(e1, nb1), b1 = e1 - s1 * nb1;
-            for (int e2 = c2 - D2; e2 <= c2 + D2; ++e2) {
-                int s2 = floordiv(e2, nb2), b2 = e2 - s2 * nb2;
-                int cell = base + (b0 * nb1 + b1) * nb2 + b2;
-                int q0 = d.cell_start[cell], q1 = d.cell_start[cell + 1];
-                if (q0 == q1) continue;
-                double sx = (double)s0 * g.h[0] + (double)s1 * g.h[3] + (double)s2 * g.h[6] - me.x;
-                double sy = (double)s0 * g.h[1] + (double)s1 * g.h[4] + (double)s2 * g.h[7] - me.y;
-                double sz = (double)s0 * g.h[2] + (double)s1 * g.h[5] + (double)s2 * g.h[8] - me.z;
-                bool home = (s0 == 0) & (s1 == 0) & (s2 == 0);
-                for (int q = q0; q < q1; q += 32) {
-                    int qq = q + lane;
-                    bool ok = false;
-                    int lj = 0;
-                    if (qq < q1) {
-                        double4 c = d.spos[qq];
-                        double rx = c.x + sx, ry = c.y + sy, rz = c.z + sz;
-                        double r2 = rx * rx + ry * ry + rz * rz;
-                        lj = (int)__double_as_longlong(c.w);
-                        ok = (r2 < R2) && !(home && qq == (int)p);
+    const int lane = threadIdx.x & 31, l = lane & 7, qg = lane >> 3;
+    const unsigned qmask = 0xffu << (8 * qg);
+    const unsigned lt = (1u << l) - 1u;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const double R2 = d.r_list2;
+    for (long long p4 = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 4; p4 < d.N; p4 += nwarps * 4) {
+        const long long p = p4 + qg;
+        if (p >= d.N) continue;
+        const int s = d.sysidx[p];           /* sorted slots of a system occupy the system's own range */
+        if (FILL && d.nbr_len[s] < 0) continue;
+        const SysGeom &g = d.geom[s];
+        const int a0 = d.sysoff[s];
+        const int base = a0 + s;
+        const double4 me = d.spos[p];
+        const int li = (int)__double_as_longlong(me.w);
+        const int lin = d.atom_cell[a0 + li] - base;
+        const int nb0 = g.nb[0], nb1 = g.nb[1], nb2 = g.nb[2];
+        const int c2 = lin % nb2, c1 = (lin / nb2) % nb1, c0 = lin / (nb2 * nb1);
+        const int D0 = g.D[0], D1 = g.D[1], D2 = g.D[2];
+        int cnt = 0;
+        const long long off = FILL ? d.nbr_off[a0 + li] : 0;
+        for (int e0 = c0 - D0; e0 <= c0 + D0; ++e0) {
+            const int s0 = floordiv(e0, nb0), b0 = e0 - s0 * nb0;
+            for (int e1 = c1 - D1; e1 <= c1 + D1; ++e1) {
+                const int s1 = floordiv(e1, nb1), b1 = e1 - s1 * nb1;
+                const double tx = (double)s0 * g.h[0] + (double)s1 * g.h[3] - me.x;
+                const double ty = (double)s0 * g.h[1] + (double)s1 * g.h[4] - me.y;
+                const double tz = (double)s0 * g.h[2] + (double)s1 * g.h[5] - me.z;
+                for (int e2 = c2 - D2; e2 <= c2 + D2; ++e2) {
+                    const int s2 = floordiv(e2, nb2), b2 = e2 - s2 * nb2;
+                    const int cell = base + (b0 * nb1 + b1) * nb2 + b2;
+                    const int q0 = d.cell_start[cell], q1 = d.cell_start[cell + 1];
+                    if (q0 == q1) continue;
+                    const double sx = tx + (double)s2 * g.h[6], sy = ty + (double)s2 * g.h[7], sz = tz + (double)s2 * g.h[8];
+                    const bool home = (s0 == 0) & (s1 == 0) & (s2 == 0);
+                    for (int q = q0; q < q1; q += 8) {
+                        const int qq = q + l;
+                        bool ok = false;
+                        int lj = 0;
+                        if (qq < q1) {
+                            const double4 c = d.spos[qq];
+                            const double rx = c.x + sx, ry = c.y + sy, rz = c.z + sz;
+                            const double r2 = rx * rx + ry * ry + rz * rz;
+                            lj = (int)__double_as_longlong(c.w);
+                            ok = (r2 < R2) && !(home && qq == (int)p);
+                        }
+                        const unsigned m = (__ballot_sync(qmask, ok) >> (8 * qg)) & 0xffu;
+                        if (FILL && ok) d.nbr[off + cnt + __popc(m & lt)] = ts_pack_nbr(lj, s0, s1, s2);
+                        cnt += __popc(m);
                     }
-                    unsigned m = __ballot_sync(0xffffffffu, ok);
-                    if (FILL && ok) d.nbr[off + cnt + __popc(m & lt)] = ts_pack_nbr(lj, s0, s1, s2);
-                    cnt += __popc(m);
                 }
             }
         }
+        if (!FILL && l == 0) d.nbr_cnt[a0 + li] = cnt;
     }
-    if (!FILL && lane == 0) d.nbr_cnt[a0 + li] = cnt;
 }
 
 __global__ void k_nbrscan(DevState d)
@@ -310,7 +318,8 @@ void launch_build(ts_state *st, bool force, cudaStream_t q)
     int tb = 256;
     int nbz = (int)((n + tb - 1) / tb); if (nbz > 148 * 8) nbz = 148 * 8;
     int nba = (int)((d.N + tb - 1) / tb);
-    long long nwarp_blocks = (d.N * 32 + tb - 1) / tb;
+    long long nwarp_blocks = (d.N * 8 + tb - 1) / tb;          /* 8 lanes per atom ... */
+    if (nwarp_blocks > 148 * 16) nwarp_blocks = 148 * 16;       /* ... in a capped, grid-stride grid */
     k_build_begin<<<nbz, tb, 0, q>>>(d);
     if (d.dtype == TS_F32) k_bin<float><<<nba, tb, 0, q>>>(d); else k_bin<double><<<nba, tb, 0, q>>>(d);
     k_cellscan<<<d.S, 256, 0, q>>>(d);

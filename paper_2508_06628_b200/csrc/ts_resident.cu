@@ -886,10 +886,11 @@ bool resident_supported(ts_state *st)
         double nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
         need = fmax(need, nbar);
         /* atoms + dummies + ghosts.  The ghosts of a bank group occupy one of eight interleaved slot sequences, so the
-         * array needs 8 x the fullest group: mean + 4 sigma of a sum of n / 8 independent image counts (a lattice
-         * written cell by cell deviates systematically by ~2.5 sigma: measured on configs[1]), + 8 per group. */
+         * array needs 8 x the fullest group: mean + 6 sigma of a sum of n / 8 independent image counts (a lattice
+         * written cell by cell deviates systematically by ~2.5 sigma: measured on configs[1]; 4 sigma overflowed a
+         * few of the 10^6 group fills of a 10^4-system liquid batch), + 8 per group. */
         const double mean_c = images - 1.0, var_c = fmax(0.0, (images2 - 2.0 * images + 1.0) - mean_c * mean_c);
-        const double per_group = mean_c * n / 8.0 + 4.0 * sqrt(var_c * n / 8.0) + 8.0;
+        const double per_group = mean_c * n / 8.0 + 6.0 * sqrt(var_c * n / 8.0) + 8.0;
         need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 8.0 * ceil(per_group));
     }
     if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
