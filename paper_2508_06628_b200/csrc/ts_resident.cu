@@ -10,7 +10,8 @@
  *                    slots: every periodic image of an atom that can lie within r_list of the cell
  *                    (the atom is within r_list of a face) owns a slot holding x + S.h.  Every owner
  *                    publishes its atom and its ghosts into every CTA of the cluster through DSMEM.
- *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only)
+ *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only; aliased onto the ghost slots,
+ *                    which are dead between the cluster barrier of a step and the ghost refresh after a rebuild)
  *     gtab[N_s]      first ghost slot, active axes and image signs of every atom (rebuilds only)
  *     rows[A][pitch] the Verlet list of the CTA's own atoms: 16-bit entries = byte offset of the
  *                    neighbour's slot.  Thanks to the ghosts EVERY pair is a plain difference of two
@@ -38,6 +39,7 @@
 #include <cooperative_groups.h>
 #include <math.h>
 #include <string.h>
+#include <stdio.h>
 #include <stdlib.h>
 
 #include <vector>
@@ -841,7 +843,10 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.CL = CL; c.A = A; c.pitch = pitch; c.NS = need_slots; c.nwarps = nwarps;
     unsigned o = 0;
     c.o_pos = o; o += up16((unsigned)(c.NS * 4 * w));
-    c.o_fr = o; o += up16((unsigned)(nmax + 16) * 16u);          /* padded: the builder tests two candidates per trip */
+    /* fr (rebuilds only; padded: the builder tests two candidates per trip) lives INSIDE the ghost part of the first
+     * position plane: a rebuild runs between the cluster barrier of a step and the ghost refresh that follows it,
+     * when no ghost slot is live; need_slots >= 2 N8 + 32 keeps it inside the array */
+    c.o_fr = c.o_pos + (unsigned)(((nmax + 7) & ~7) + 8) * 16u;
     c.o_gtab = o; o += up16((unsigned)nmax * 4u);
     c.o_rows = o; o += up16((unsigned)A * (unsigned)pitch * 2u);
     c.o_fs = o; o += up16((unsigned)(3 * A * w));
@@ -886,52 +891,67 @@ bool resident_supported(ts_state *st)
         double nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
         need = fmax(need, nbar);
         /* atoms + dummies + ghosts.  The ghosts of a bank group occupy one of eight interleaved slot sequences, so the
-         * array needs 8 x the fullest group: mean + 6 sigma of a sum of n / 8 independent image counts (a lattice
-         * written cell by cell deviates systematically by ~2.5 sigma: measured on configs[1]; 4 sigma overflowed a
-         * few of the 10^6 group fills of a 10^4-system liquid batch), + 8 per group. */
+         * array needs 8 x the fullest group: mean + z sigma of a sum of n / 8 independent image counts, + 8 per group.
+         * z = 6: 4 sigma overflowed a few of the 10^6 group fills of a 10^4-system liquid batch; a lattice written cell
+         * by cell deviates systematically by ~2.5 sigma (measured on configs[1]).  An overflow is always detected and
+         * flagged (TS_FLAG_NBR_OVERFLOW), never silent. */
         const double mean_c = images - 1.0, var_c = fmax(0.0, (images2 - 2.0 * images + 1.0) - mean_c * mean_c);
-        const double per_group = mean_c * n / 8.0 + 6.0 * sqrt(var_c * n / 8.0) + 8.0;
-        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 8.0 * ceil(per_group));
+        const double sd_g = sqrt(var_c * n / 8.0);
+        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 8.0 * ceil(mean_c * n / 8.0 + 6.0 * sd_g + 8.0));
     }
     if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
-    int ns = (((int)ceil(need_slots) + 7) / 8) * 8;
-    if (getenv("TS_RES_NS")) ns = atoi(getenv("TS_RES_NS"));
-    if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
-    if (ns < ((nmax + 7) & ~7) + 16) return false;
     double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
     int need_row = (int)ceil(need * slack);
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    ResCfg best; bool have = false;
-    const char *force_cl = getenv("TS_RES_CL");
-    for (int CL = 1; CL <= 8; CL *= 2) {
-        ResCfg c;
-        memset(&c, 0, sizeof c);
-        if (force_cl && atoi(force_cl) != CL) continue;
-        if (!res_layout(c, CL, nmax, need_row, ns, d.dtype, d.n_types)) continue;
-        best = c; have = true;
-        if ((long long)S * CL >= (nsm * 3) / 4 || c.A <= 64) break;   /* enough CTAs to occupy the chip */
-    }
-    if (!have) return false;
-    best.eps_rel = eps_rel;
     ResKernel k = pick_kernel(st);
-    if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)best.smem) != cudaSuccess) {
-        cudaGetLastError();
-        return false;
-    }
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof lc);
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)best.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    lc.gridDim = dim3((unsigned)(best.CL * S)); lc.blockDim = dim3((unsigned)(best.nwarps * 32));
-    lc.dynamicSmemBytes = best.smem; lc.attrs = at; lc.numAttrs = 1;
+    const char *force_cl = getenv("TS_RES_CL");
+    /* launch shape for a given slot count: smallest cluster that fits and fills the chip; cost ~ waves x per-CTA work */
+    auto plan = [&](double slots, ResCfg &out, int &maxc_out, double &cost) -> bool {
+        int ns = (((int)ceil(slots) + 7) / 8) * 8;
+        if (getenv("TS_RES_NS")) ns = atoi(getenv("TS_RES_NS"));
+        if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
+        if (ns < 2 * ((nmax + 7) & ~7) + 32) ns = 2 * ((nmax + 7) & ~7) + 32;     /* room for fr inside the ghost part */
+        bool have = false;
+        for (int CL = 1; CL <= 8; CL *= 2) {
+            ResCfg c;
+            memset(&c, 0, sizeof c);
+            if (force_cl && atoi(force_cl) != CL) continue;
+            if (!res_layout(c, CL, nmax, need_row, ns, d.dtype, d.n_types)) continue;
+            out = c; have = true;
+            if ((long long)S * CL >= (nsm * 3) / 4 || c.A <= 64) break;   /* enough CTAs to occupy the chip */
+        }
+        if (!have) return false;
+        if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)out.smem) != cudaSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        cudaLaunchConfig_t lc;
+        memset(&lc, 0, sizeof lc);
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)out.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        lc.gridDim = dim3((unsigned)(out.CL * S)); lc.blockDim = dim3((unsigned)(out.nwarps * 32));
+        lc.dynamicSmemBytes = out.smem; lc.attrs = at; lc.numAttrs = 1;
+        int maxc = 0;
+        if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
+            cudaGetLastError();
+            return false;
+        }
+        maxc_out = maxc;
+        const int live = S < maxc ? S : maxc;
+        cost = (double)((S + live - 1) / live) * ((double)out.A + 40.0 * out.CL);
+        return true;
+    };
+    ResCfg best;
     int maxc = 0;
-    if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
-        cudaGetLastError();
-        return false;
-    }
+    double cost = 0.0;
+    if (!plan(need_slots, best, maxc, cost)) return false;
+    best.eps_rel = eps_rel;
+    if (getenv("TS_RES_VERBOSE"))
+        fprintf(stderr, "[ts resident] CL %d A %d pitch %d NS %d warps %d smem %u clusters %d of %d systems\n", best.CL, best.A,
+                best.pitch, best.NS, best.nwarps, best.smem, S < maxc ? S : maxc, S);
     best.n_clusters = S < maxc ? S : maxc;
     p->cfg = best;
     p->ok = true;
