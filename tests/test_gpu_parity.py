@@ -201,3 +201,23 @@ def test_fp32_baoab_noise_follows_the_oracle_stream(ts, orc, engine):
     assert dv.max() <= 2e-7
     assert np.abs(st.numpy("pos").astype(np.float64) - o["pos"]).max() <= 2e-5
     st.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_nve_binary_soft_sphere_fp64(ts, orc, engine):
+    """Two atom types (per-pair parameter table) under MD: the resident engine's generic, multi-type pair path and the
+    general engine against the oracle (the cfg4 mixture, here with velocities and velocity Verlet instead of FIRE)."""
+    b = wl.cfg4(range(5), n_atoms=200)
+    rng = np.random.Generator(np.random.PCG64(12345))
+    b = wl.with_(b, vel=rng.normal(0.0, 0.3, size=b.vel.shape))
+    md = dict(integrator="nve", dt=0.004, temperature=0.0, friction=0.0, seed=0)
+    o = orc.md_run(b, "nve", md["dt"], 60)
+    st = ts.SimState(b, engine=engine)
+    st.md_step(md, 60, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == engine
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.abs(st.numpy("force") - o["F"]).max() <= 1e-8
+    assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-9)
+    assert np.abs(st.numpy("virial") - o["W"]).max() <= 1e-8 * np.abs(o["W"]).max()
+    st.close()
