@@ -8,9 +8,9 @@
  *   k_cellscan    : per-system exclusive scan of the cell counters (block per system; the key
  *                   space of system s is [sysoff[s]+s, sysoff[s+1]+s] so no global scan exists)
  *   k_scatter     : counting-sort scatter of wrapped fp64 coordinates; x_ref and pos4 refresh
- *   k_nbr<0>      : warp-cooperative scan of the (2D+1)^3 extended-bin stencil, COUNT
- *   k_nbrscan     : per-system exclusive scan of the counts + capacity check (overflow flag)
- *   k_nbr<1>      : same scan, FILL of the CSR rows (skipped for overflowed systems)
+ *   k_nbr_fill    : quarter-warp walk of the (2D+1)^3 extended-bin stencil, rows buffered in shared memory,
+ *                   reserved in the system's CSR segment with one atomicAdd and copied out (ONE pass)
+ *   k_nbr_finish  : cursor > capacity -> overflow state (flag, nothing was written past capacity)
  * The cutoff test is strict r^2 < r_list^2 in fp64 on the promoted coordinates (R9, R27).
  */
 #include "ts_internal.cuh"
@@ -73,6 +73,8 @@ __global__ void k_build_begin(DevState d)
     long long n = d.N + d.S + 1;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
         d.cell_count[i] = 0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < d.S; i += (long long)gridDim.x * blockDim.x)
+        d.nbr_len[i] = 0;                     /* row cursor of the system's CSR segment (k_nbr_fill) */
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         d.status->nnz = 0ull;
         d.status->max_nbr = 0u;
@@ -194,24 +196,33 @@ __global__ void k_scatter(DevState d)
 
 __device__ __forceinline__ int floordiv(int a, int n) { int q = a / n; return (a % n < 0) ? q - 1 : q; }
 
-/* One quarter-warp (8 lanes) per sorted slot p, four consecutive slots per warp: sorted slots that follow each other
- * sit in the same or in adjacent bins, so the four stencil walks of a warp stay converged and share their loads.  The
- * lanes of a quarter stride over the atoms of each stencil bin; hits are compacted with a quarter-wide ballot.  The
- * grid is capped (grid-stride over the slots): when no rebuild is due the launch costs a few microseconds. */
-template <int FILL>
-__global__ void __launch_bounds__(256) k_nbr(DevState d)
+/* Neighbour search, ONE pass.  One quarter-warp (8 lanes) per sorted slot p, four consecutive slots per warp: sorted
+ * slots that follow each other sit in the same or in adjacent bins, so the four stencil walks of a warp stay converged
+ * and share their loads.  The lanes of a quarter stride over the atoms of each stencil bin; hits are compacted with a
+ * quarter-wide ballot into a shared-memory buffer (NBR_BUF entries per atom).  When the walk is done the quarter
+ * reserves a contiguous row inside the CSR segment of its system with one atomicAdd on the system's cursor (nbr_len)
+ * and copies the row out: no counting pass, no scan.  Rows of a system are therefore stored in arrival order (nbr_off
+ * says where); the content and order of every row are deterministic.  Nothing is written past the capacity of the
+ * segment: a row that does not fit only advances the cursor, and k_nbr_finish turns cursor > capacity into the
+ * overflow state (nbr_len = -1, TS_FLAG_NBR_OVERFLOW).  The grid is capped (grid-stride over the slots): when no
+ * rebuild is due the launch costs a few microseconds. */
+#define NBR_BUF 256
+__global__ void __launch_bounds__(256) k_nbr_fill(DevState d)
 {
     if (!d.status->need_rebuild) return;
+    __shared__ unsigned buf[32 * NBR_BUF];
     const int lane = threadIdx.x & 31, l = lane & 7, qg = lane >> 3;
+    unsigned *const mybuf = buf + (size_t)(threadIdx.x >> 3) * NBR_BUF;
     const unsigned qmask = 0xffu << (8 * qg);
     const unsigned lt = (1u << l) - 1u;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
     const double R2 = d.r_list2;
+    unsigned long long nnz = 0ull;
+    unsigned mx = 0u;
     for (long long p4 = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 4; p4 < d.N; p4 += nwarps * 4) {
         const long long p = p4 + qg;
         if (p >= d.N) continue;
         const int s = d.sysidx[p];           /* sorted slots of a system occupy the system's own range */
-        if (FILL && d.nbr_len[s] < 0) continue;
         const SysGeom &g = d.geom[s];
         const int a0 = d.sysoff[s];
         const int base = a0 + s;
@@ -222,7 +233,6 @@ __global__ void __launch_bounds__(256) k_nbr(DevState d)
         const int c2 = lin % nb2, c1 = (lin / nb2) % nb1, c0 = lin / (nb2 * nb1);
         const int D0 = g.D[0], D1 = g.D[1], D2 = g.D[2];
         int cnt = 0;
-        const long long off = FILL ? d.nbr_off[a0 + li] : 0;
         for (int e0 = c0 - D0; e0 <= c0 + D0; ++e0) {
             const int s0 = floordiv(e0, nb0), b0 = e0 - s0 * nb0;
             for (int e1 = c1 - D1; e1 <= c1 + D1; ++e1) {
@@ -249,49 +259,55 @@ __global__ void __launch_bounds__(256) k_nbr(DevState d)
                             ok = (r2 < R2) && !(home && qq == (int)p);
                         }
                         const unsigned m = (__ballot_sync(qmask, ok) >> (8 * qg)) & 0xffu;
-                        if (FILL && ok) d.nbr[off + cnt + __popc(m & lt)] = ts_pack_nbr(lj, s0, s1, s2);
+                        const int at = cnt + __popc(m & lt);
+                        if (ok && at < NBR_BUF) mybuf[at] = ts_pack_nbr(lj, s0, s1, s2);
                         cnt += __popc(m);
                     }
                 }
             }
         }
-        if (!FILL && l == 0) d.nbr_cnt[a0 + li] = cnt;
+        /* reserve the row and copy it out */
+        long long start = 0;
+        if (l == 0) {
+            const unsigned long long want = cnt <= NBR_BUF ? (unsigned long long)cnt : (1ull << 40);   /* too long for the buffer: overflow */
+            start = (long long)atomicAdd((unsigned long long *)&d.nbr_len[s], want);
+        }
+        start = __shfl_sync(qmask, start, 8 * qg);
+        const long long seg = d.nbr_base[s], cap = d.nbr_base[s + 1] - seg;
+        __syncwarp(qmask);
+        if (cnt <= NBR_BUF && start + cnt <= cap)
+            for (int k = l; k < cnt; k += 8) d.nbr[seg + start + k] = mybuf[k];
+        __syncwarp(qmask);
+        if (l == 0) {
+            d.nbr_off[a0 + li] = seg + start;
+            d.nbr_cnt[a0 + li] = cnt;
+            nnz += (unsigned long long)cnt;
+            mx = max(mx, (unsigned)cnt);
+        }
+    }
+    /* statistics: one atomic per warp */
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nnz += __shfl_xor_sync(0xffffffffu, nnz, o);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if (lane == 0 && nnz) {
+        atomicAdd(&d.status->nnz, nnz);
+        atomicMax(&d.status->max_nbr, mx);
     }
 }
 
-__global__ void k_nbrscan(DevState d)
+/* cursor -> state of the segment: pairs in use, or -1 when the rows did not fit (overflow: flagged, list invalid) */
+__global__ void k_nbr_finish(DevState d)
 {
     if (!d.status->need_rebuild) return;
-    __shared__ long long sh[33];
-    __shared__ int shm[32];
-    int s = blockIdx.x;
-    int a0 = d.sysoff[s], a1 = d.sysoff[s + 1];
-    long long base = d.nbr_base[s], cap = d.nbr_base[s + 1] - base;
-    long long run = 0;
-    int mx = 0;
-    for (int i0 = a0; i0 < a1; i0 += blockDim.x) {
-        int i = i0 + threadIdx.x;
-        long long v = i < a1 ? (long long)d.nbr_cnt[i] : 0;
-        mx = max(mx, (int)v);
-        long long tot;
-        long long ex = block_excl_scan<long long>(v, sh, &tot);
-        if (i < a1) d.nbr_off[i] = base + run + ex;
-        run += tot;
-    }
-    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    if ((threadIdx.x & 31) == 0) shm[threadIdx.x >> 5] = mx;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mx = max(mx, shm[w]);
-        atomicMax(&d.status->max_nbr, (unsigned)mx);
-        atomicAdd(&d.status->nnz, (unsigned long long)run);
-        if (run > cap) {
-            d.nbr_len[s] = -1;
-            atomicOr(&d.status->flags, TS_FLAG_NBR_OVERFLOW);
-            d.status->list_valid = 0u;
-        } else {
-            d.nbr_len[s] = run;
-        }
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= d.S) return;
+    const long long cap = d.nbr_base[s + 1] - d.nbr_base[s];
+    if (d.nbr_len[s] > cap) {
+        d.nbr_len[s] = -1;
+        atomicOr(&d.status->flags, TS_FLAG_NBR_OVERFLOW);
+        d.status->list_valid = 0u;
     }
 }
 
@@ -324,10 +340,9 @@ void launch_build(ts_state *st, bool force, cudaStream_t q)
     if (d.dtype == TS_F32) k_bin<float><<<nba, tb, 0, q>>>(d); else k_bin<double><<<nba, tb, 0, q>>>(d);
     k_cellscan<<<d.S, 256, 0, q>>>(d);
     if (d.dtype == TS_F32) k_scatter<float><<<nba, tb, 0, q>>>(d); else k_scatter<double><<<nba, tb, 0, q>>>(d);
-    k_nbr<0><<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
-    k_nbrscan<<<d.S, 256, 0, q>>>(d);
-    k_nbr<1><<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
+    k_nbr_fill<<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
+    k_nbr_finish<<<(d.S + 255) / 256, 256, 0, q>>>(d);
     k_build_end<<<1, 1, 0, q>>>(d);
-    st->launches += 8;
+    st->launches += 7;
     st->list_built = true;
 }
