@@ -22,7 +22,8 @@ __device__ __forceinline__ int type_of(const typename Vec4<T>::type &q)
     return (int)__double_as_longlong((double)q.w);
 }
 
-template <typename T, int KIND, bool EV>
+/* EV = 0: forces only; 1: + energy (FIRE: the virial accumulators would cost 12 registers of occupancy); 2: + virial */
+template <typename T, int KIND, int EV>
 __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
 {
     typedef typename Vec4<T>::type V4;
@@ -67,9 +68,11 @@ __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
                 g = in ? g : (T)0; V = in ? V : (T)0;
                 fx += g * rx; fy += g * ry; fz += g * rz;
                 e += V;
-                T gx = g * rx, gy = g * ry;
-                w0 += gx * rx; w1 += gx * ry; w2 += gx * rz;
-                w3 += gy * ry; w4 += gy * rz; w5 += g * rz * rz;
+                if (EV == 2) {
+                    T gx = g * rx, gy = g * ry;
+                    w0 += gx * rx; w1 += gx * ry; w2 += gx * rz;
+                    w3 += gy * ry; w4 += gy * rz; w5 += g * rz * rz;
+                }
             } else {
                 T g = pot_force<T, KIND>(pe, r2);
                 g = in ? g : (T)0;
@@ -91,6 +94,7 @@ __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
     }
     if (EV) {
         /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
+        constexpr int NQ = EV == 2 ? 7 : 1;
         double acc[7] = { 0.5 * (double)e, -0.5 * (double)w0, -0.5 * (double)w1, -0.5 * (double)w2,
                           -0.5 * (double)w3, -0.5 * (double)w4, -0.5 * (double)w5 };
         int key = act ? s : -1;
@@ -99,12 +103,12 @@ __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
         bool whole = __all_sync(FULL, key == sl) && sl >= 0;
         if (whole) {
 #pragma unroll
-            for (int q = 0; q < 7; ++q)
+            for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
             if ((threadIdx.x & 31) == 0) {
                 atomicAdd(&d.energy[sl], acc[0]);
-                if (d.virial) {
+                if (EV == 2 && d.virial) {
                     double *W = d.virial + 9 * (size_t)sl;
                     atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
                     atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
@@ -113,12 +117,12 @@ __global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
             }
         } else {
 #pragma unroll
-            for (int q = 0; q < 7; ++q)
+            for (int q = 0; q < NQ; ++q)
 #pragma unroll
                 for (int o = 1; o < LPA; o <<= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
             if (act && sub == 0) {
                 atomicAdd(&d.energy[s], acc[0]);
-                if (d.virial) {
+                if (EV == 2 && d.virial) {
                     double *W = d.virial + 9 * (size_t)s;
                     atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
                     atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
@@ -150,10 +154,11 @@ static void launch_pair_k(ts_state *st, unsigned want, bool masked, cudaStream_t
     if (want) {
         if (!(want & TS_WANT_VIRIAL)) d.virial = nullptr;
         k_zero_ev<<<(d.S + 127) / 128, 128, 0, q>>>(d, masked ? 1 : 0, want);
-        k_pair<T, KIND, true><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        if (d.virial) k_pair<T, KIND, 2><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        else k_pair<T, KIND, 1><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
         st->launches += 2;
     } else {
-        k_pair<T, KIND, false><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        k_pair<T, KIND, 0><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
         st->launches += 1;
     }
 }
