@@ -24,7 +24,7 @@ __device__ __forceinline__ int type_of(const typename Vec4<T>::type &q)
 
 /* EV = 0: forces only; 1: + energy (FIRE: the virial accumulators would cost 12 registers of occupancy); 2: + virial */
 template <typename T, int KIND, int EV>
-__global__ void __launch_bounds__(256) k_pair(DevState d, int masked)
+__global__ void __launch_bounds__(256, 3) k_pair(DevState d, int masked)
 {
     typedef typename Vec4<T>::type V4;
     const unsigned FULL = 0xffffffffu;
