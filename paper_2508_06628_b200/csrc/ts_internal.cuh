@@ -157,6 +157,7 @@ bool resident_supported(ts_state *st);
 void resident_invalidate(ts_state *st);
 void resident_free(ts_state *st);
 ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q);
+ts_status resident_fire(ts_state *st, const ts_fire_params &fp, int n_steps, cudaStream_t q);
 
 /* ------------------------------------------------------------------ device helpers */
 template <typename T> struct Vec4;

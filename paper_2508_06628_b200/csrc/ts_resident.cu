@@ -63,7 +63,7 @@ struct ResCfg {
     int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
-    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc;
+    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc, o_fire;
     unsigned smem;
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
 };
@@ -597,9 +597,48 @@ __device__ __forceinline__ double reduce8(cg::cluster_group &cluster, int CL, in
     return s;
 }
 
+/* ------------------------------------------------------------------ FIRE inside the resident engine (O6, R21, R22)
+ * The per-system FIRE state lives in shared memory, replicated in every CTA of the cluster: each CTA runs the same
+ * state machine on the same (bitwise identical) reduced values, so no state is ever sent. */
+struct FireSm {
+    double dt, alpha;
+    int npos, nsteps, status, pad;
+    double acc[4];     /* max |F_i|^2, P = F.v, v.v, F.F of the system */
+};
+
+/* max / sums over the system in fixed order: warp shuffle -> per-warp slots -> per-CTA -> every CTA of the cluster */
+__device__ __forceinline__ void fire_reduce(cg::cluster_group &cluster, int CL, int rank, double f2, double P, double vv,
+                                            double *red, double *cred, int nwarps, double out[4])
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double mx = f2, ff = f2;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        P += __shfl_xor_sync(0xffffffffu, P, o);
+        vv += __shfl_xor_sync(0xffffffffu, vv, o);
+        ff += __shfl_xor_sync(0xffffffffu, ff, o);
+    }
+    if (lane == 0) { red[warp * 8 + 0] = mx; red[warp * 8 + 1] = P; red[warp * 8 + 2] = vv; red[warp * 8 + 3] = ff; }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double a = red[threadIdx.x];
+        for (int w = 1; w < nwarps; ++w) a = threadIdx.x == 0 ? fmax(a, red[w * 8]) : a + red[w * 8 + threadIdx.x];
+        for (int r = 0; r < CL; ++r) cluster.map_shared_rank(cred, r)[rank * 8 + threadIdx.x] = a;
+    }
+    if (CL > 1) cluster.sync(); else __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        double a = cred[k];
+        for (int r = 1; r < CL; ++r) a = k == 0 ? fmax(a, cred[r * 8 + k]) : a + cred[r * 8 + k];
+        out[k] = a;
+    }
+    if (CL > 1) cluster.sync(); else __syncthreads();          /* cred may be rewritten by the next reduction */
+}
+
 /* ------------------------------------------------------------------ the kernel */
-template <typename T, int KIND, bool NT1>
-__global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THREADS_F64, 1) k_resident_md(DevState d, MdConst c, ResCfg rc, int n_steps, unsigned want)
+template <typename T, int KIND, bool NT1, bool FIRE>
+__global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THREADS_F64, 1) k_resident_md(DevState d, MdConst c, ResCfg rc, int n_steps, unsigned want, ts_fire_params fp)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     cg::cluster_group cluster = cg::this_cluster();
@@ -622,6 +661,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     T *gh = (T *)(misc + 1);            /* h[9], hinv[9] in the state dtype */
     float *G = (float *)(gh + 18);      /* metric of the fixed-point fractions, [6] + rb2 */
     unsigned *thr = (unsigned *)(G + 8);/* ghost thresholds [3] */
+    FireSm *fsm = (FireSm *)(smem + rc.o_fire);
+    double *fred = (double *)(fsm + 1);   /* per-warp scratch of fire_reduce, [nwarps][8] */
 
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
@@ -634,6 +675,11 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const int a_begin = rank * A_s;
         const int A_own = max(0, min(A_s, N_s - a_begin));
         const SysGeom &geo = d.geom[s];
+        int fstat0 = 0;
+        if (FIRE) {                                    /* finished systems stay bit-unchanged (R22) */
+            fstat0 = d.f_status[s];
+            if (fstat0 == TS_FIRE_CONVERGED || fstat0 == TS_FIRE_FAILED) continue;
+        }
         /* ---- per-system constants into shared memory */
         if (tid < 9) { gh[tid] = (T)geo.h[tid]; gh[9 + tid] = (T)geo.hinv[tid]; }
         if (tid == 64) {
@@ -655,6 +701,14 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 thr[k] = rho >= 0.5 ? 0x80000000u : (unsigned)(rho * 4294967296.0);
             }
             misc->flags[0] = 0; misc->flags[1] = 0; misc->nnz = 0u; misc->rebuilds = 0u; misc->overflow = 0;
+            if (FIRE) {
+                const bool fresh = fstat0 == TS_FIRE_FRESH;
+                fsm->dt = fresh ? fp.dt_start : d.f_dt[s];
+                fsm->alpha = fresh ? fp.alpha_start : d.f_alpha[s];
+                fsm->npos = fresh ? 0 : d.f_npos[s];
+                fsm->nsteps = fresh ? 0 : d.f_nsteps[s];
+                fsm->status = TS_FIRE_RUNNING;
+            }
         }
         /* ---- owner state */
         const bool own = tid < A_own;
@@ -670,10 +724,13 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             mass = ((const T *)d.mass)[gi];
             im = (T)1 / (mass * (T)d.mass_conv);
             ty = d.type[gi];
+            if (FIRE && fstat0 == TS_FIRE_FRESH) { v0 = 0; v1 = 0; v2 = 0; }
         }
         const unsigned uid = d.uid_own[s];
         const unsigned long long step0 = d.sys_step[s];
-        const T hdt = (T)c.hdt, dt = (T)c.dt;
+        T hdt = (T)c.hdt, dt = (T)c.dt;
+        int n_done = 0;                               /* steps taken by this system in this call */
+        bool have_ev = false;                         /* the last pair pass also produced E (and W) */
         cluster.sync();                               /* constants visible; previous system fully retired everywhere */
 
 #ifdef TS_RES_TIMING
@@ -681,11 +738,19 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
 #endif
         for (int n = 0; n <= n_steps; ++n) {
             const int nb = n & 1;
+            if (FIRE && n > 0) {
+                if (fsm->nsteps >= fp.max_steps) {     /* reported as failed, never counted (R24) */
+                    __syncthreads();
+                    if (tid == 0) fsm->status = TS_FIRE_FAILED;
+                    break;
+                }
+                dt = (T)fsm->dt; hdt = (T)0.5 * dt;
+            }
             if (n > 0) {
                 bool moved = false;
                 if (own) {
                     /* first half of the step (O3 / O4), as in the general engine */
-                    if (c.integrator == TS_NVE) {
+                    if (FIRE || c.integrator == TS_NVE) {
                         v0 = v0 + hdt * (f0 * im); x0 = x0 + dt * v0;
                         v1 = v1 + hdt * (f1 * im); x1 = x1 + dt * v1;
                         v2 = v2 + hdt * (f2 * im); x2 = x2 + dt * v2;
@@ -705,7 +770,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
                 }
                 TICK(0);
-                cl_wait();                            /* every CTA of the cluster has finished reading the old positions */
+                if (!FIRE) cl_wait();                 /* every CTA of the cluster has finished reading the old positions (FIRE: fire_reduce's barriers) */
                 TICK(1);
                 if (own) {
                     if (moved)
@@ -758,16 +823,68 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             const bool last = n == n_steps;
             if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
             else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
+            have_ev = last;
             TICK(8);
-            cl_arrive_relaxed();                      /* this CTA no longer reads the positions of step n */
+            if (!FIRE) cl_arrive_relaxed();           /* this CTA no longer reads the positions of step n */
             __syncthreads();
             TICK(9);
             if (own) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
                 if (n > 0) { v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im); }
             }
+            if (n > 0) n_done = n;
+            if (FIRE) {
+                /* the four per-system reductions, then the FIRE state machine (identical in every CTA) */
+                double fsq = 0.0, P = 0.0, vv = 0.0;
+                if (own) {
+                    fsq = (double)f0 * (double)f0 + (double)f1 * (double)f1 + (double)f2 * (double)f2;
+                    P = (double)f0 * (double)v0 + (double)f1 * (double)v1 + (double)f2 * (double)v2;
+                    vv = (double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2;
+                }
+                double a[4];
+                fire_reduce(cluster, CL, rank, fsq, P, vv, fred, cred, rc.nwarps, a);
+                const bool conv = sqrt(a[0]) < fp.f_max;
+                if (n == 0) {                         /* fresh system: the 0-step convergence test */
+                    if (conv && fstat0 == TS_FIRE_FRESH) { if (tid == 0) fsm->status = TS_FIRE_CONVERGED; break; }
+                } else {
+                    const double al = fsm->alpha;     /* mixing uses alpha before its update (R21) */
+                    if (!conv) {
+                        if (a[1] > 0.0) {
+                            const double fn = sqrt(a[3]), vn = sqrt(a[2]);
+                            if (fn > 0.0 && own) {
+                                const T cf = (T)(al * (vn / fn)), om = (T)(1.0 - al);
+                                v0 = om * v0 + cf * f0; v1 = om * v1 + cf * f1; v2 = om * v2 + cf * f2;
+                            }
+                        } else if (own) { v0 = 0; v1 = 0; v2 = 0; }
+                    }
+                    __syncthreads();                  /* everybody has read the state of this step */
+                    if (tid == 0) {
+                        fsm->nsteps += 1;
+                        if (conv) fsm->status = TS_FIRE_CONVERGED;
+                        else if (a[1] > 0.0) {
+                            const int np = fsm->npos + 1;
+                            fsm->npos = np;
+                            if (np > fp.n_min) {
+                                const double nd = fsm->dt * fp.f_inc;
+                                fsm->dt = nd < fp.dt_max ? nd : fp.dt_max;
+                                fsm->alpha = fsm->alpha * fp.f_alpha;
+                            }
+                        } else {
+                            fsm->dt = fsm->dt * fp.f_dec;
+                            fsm->alpha = fp.alpha_start;
+                            fsm->npos = 0;
+                        }
+                    }
+                    __syncthreads();
+                    if (conv) break;                  /* frozen at the first step whose new forces satisfy the criterion */
+                }
+            }
         }
-        cl_wait();                                    /* pairs the last arrive */
+        if (!FIRE) cl_wait();                         /* pairs the last arrive */
+        if (FIRE && !have_ev) {                       /* stopped before the last pass: E of the final positions */
+            pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
+            __syncthreads();
+        }
 #ifdef TS_RES_TIMING
         if (tid == 0) for (int k = 0; k < 12; ++k) atomicAdd(&g_res_prof[k], (unsigned long long)prof_acc[k]);
 #endif
@@ -782,7 +899,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const double tot = reduce8(cluster, CL, rank, ke, red, cred, rc.nwarps);
         if (rank == 0 && tid < 8) {
             if (tid == 0) d.energy[s] = tot;
-            if (tid == 7) d.kinetic[s] = tot;
+            if (tid == 7 && !FIRE) d.kinetic[s] = tot;
             if (tid >= 1 && tid <= 6 && (want & TS_WANT_VIRIAL)) {
                 /* acc order: xx xy xz yy yz zz -> symmetric 3x3 */
                 const int at[6][2] = { { 0, 0 }, { 1, 3 }, { 2, 6 }, { 4, 4 }, { 5, 7 }, { 8, 8 } };
@@ -796,7 +913,12 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             atomicAdd(&d.status->res_nnz, (unsigned long long)misc->nnz);
             if (rank == 0) {
                 atomicAdd(&d.status->res_rebuilds, (unsigned long long)misc->rebuilds);
-                d.sys_step[s] = step0 + (unsigned long long)n_steps;
+                d.sys_step[s] = step0 + (unsigned long long)(FIRE ? n_done : n_steps);
+                if (FIRE) {
+                    d.f_dt[s] = fsm->dt; d.f_alpha[s] = fsm->alpha; d.f_npos[s] = fsm->npos; d.f_nsteps[s] = fsm->nsteps;
+                    d.f_status[s] = fsm->status;
+                    d.sys_active[s] = fsm->status == TS_FIRE_RUNNING ? 1 : 0;
+                }
             }
         }
         cluster.sync();                               /* nobody overwrites shared state a peer still reads */
@@ -807,22 +929,24 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
 struct ResPlan {
     bool checked, ok;
     ResCfg cfg;
+    int fire_clusters;     /* clusters in flight of the FIRE kernel (0 = not asked yet) */
 };
 static ResPlan *plan_of(ts_state *st) { return (ResPlan *)st->res_plan; }
 
-typedef void (*ResKernel)(DevState, MdConst, ResCfg, int, unsigned);
+typedef void (*ResKernel)(DevState, MdConst, ResCfg, int, unsigned, ts_fire_params);
 
-template <typename T>
+template <typename T, bool FIRE>
 static ResKernel pick_kernel_t(int kind, bool nt1)
 {
-    if (kind == TS_LJ) return nt1 ? k_resident_md<T, TS_LJ, true> : k_resident_md<T, TS_LJ, false>;
-    if (kind == TS_MORSE) return nt1 ? k_resident_md<T, TS_MORSE, true> : k_resident_md<T, TS_MORSE, false>;
-    return nt1 ? k_resident_md<T, TS_SOFT_SPHERE, true> : k_resident_md<T, TS_SOFT_SPHERE, false>;
+    if (kind == TS_LJ) return nt1 ? k_resident_md<T, TS_LJ, true, FIRE> : k_resident_md<T, TS_LJ, false, FIRE>;
+    if (kind == TS_MORSE) return nt1 ? k_resident_md<T, TS_MORSE, true, FIRE> : k_resident_md<T, TS_MORSE, false, FIRE>;
+    return nt1 ? k_resident_md<T, TS_SOFT_SPHERE, true, FIRE> : k_resident_md<T, TS_SOFT_SPHERE, false, FIRE>;
 }
-static ResKernel pick_kernel(const ts_state *st)
+static ResKernel pick_kernel(const ts_state *st, bool fire = false)
 {
     bool nt1 = st->d.n_types == 1;
-    return st->d.dtype == TS_F32 ? pick_kernel_t<float>(st->d.kind, nt1) : pick_kernel_t<double>(st->d.kind, nt1);
+    if (fire) return st->d.dtype == TS_F32 ? pick_kernel_t<float, true>(st->d.kind, nt1) : pick_kernel_t<double, true>(st->d.kind, nt1);
+    return st->d.dtype == TS_F32 ? pick_kernel_t<float, false>(st->d.kind, nt1) : pick_kernel_t<double, false>(st->d.kind, nt1);
 }
 
 static unsigned up16(unsigned x) { return (x + 15u) & ~15u; }
@@ -855,6 +979,7 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.o_red = o; o += (unsigned)(RES_MAX_THREADS / 32) * 64u;
     c.o_cred = o; o += 8u * 64u;
     c.o_misc = o; o += up16((unsigned)(sizeof(ResMisc) + 18 * w + 8 * sizeof(float) + 4 * sizeof(unsigned)));
+    c.o_fire = o; o += up16((unsigned)(sizeof(FireSm) + (RES_MAX_THREADS / 32) * 64u));
     c.smem = o;
     return o <= RES_SMEM_LIMIT;
 }
@@ -865,7 +990,7 @@ bool resident_supported(ts_state *st)
     if (!st->res_plan) st->res_plan = calloc(1, sizeof(ResPlan));
     ResPlan *p = plan_of(st);
     if (p->checked) return p->ok;
-    p->checked = true; p->ok = false;
+    p->checked = true; p->ok = false; p->fire_clusters = 0;
     const DevState &d = st->d;
     int S = d.S;
     std::vector<SysGeom> geo((size_t)S);
@@ -908,7 +1033,7 @@ bool resident_supported(ts_state *st)
     ResKernel k = pick_kernel(st);
     const char *force_cl = getenv("TS_RES_CL");
     /* launch shape for a given slot count: smallest cluster that fits and fills the chip; cost ~ waves x per-CTA work */
-    auto plan = [&](double slots, ResCfg &out, int &maxc_out, double &cost) -> bool {
+    auto plan = [&](double slots, int need_row, ResCfg &out, int &maxc_out, double &cost) -> bool {
         int ns = (((int)ceil(slots) + 7) / 8) * 8;
         if (getenv("TS_RES_NS")) ns = atoi(getenv("TS_RES_NS"));
         if (ns > RES_MAX_SLOTS) ns = RES_MAX_SLOTS & ~7;
@@ -944,10 +1069,21 @@ bool resident_supported(ts_state *st)
         cost = (double)((S + live - 1) / live) * ((double)out.A + 40.0 * out.CL);
         return true;
     };
-    ResCfg best;
-    int maxc = 0;
-    double cost = 0.0;
-    if (!plan(need_slots, best, maxc, cost)) return false;
+    /* Row capacity.  slack x the mean count is enough for a crystal or an equilibrium liquid; a configuration with
+     * ideal-gas density fluctuations (cfg4's uniformly random starting points) has Poisson counts: mean + 6 sqrt(mean)
+     * + 8.  The Poisson capacity is taken whenever it does not make the launch shape costlier (cluster size, waves);
+     * either way a row overflow is detected and flagged, never silent. */
+    const int need_row_p = (int)ceil(fmax(need * slack, need + 6.0 * sqrt(need) + 8.0));
+    ResCfg best, alt;
+    int maxc = 0, maxc_p = 0;
+    double cost = 0.0, cost_p = 0.0;
+    const bool ok0 = plan(need_slots, need_row, best, maxc, cost), okp = plan(need_slots, need_row_p, alt, maxc_p, cost_p);
+    if (!ok0 && !okp) return false;
+    if (okp && (!ok0 || cost_p <= 1.05 * cost)) { best = alt; maxc = maxc_p; }
+    if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)best.smem) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
     best.eps_rel = eps_rel;
     if (getenv("TS_RES_VERBOSE"))
         fprintf(stderr, "[ts resident] CL %d A %d pitch %d NS %d warps %d smem %u clusters %d of %d systems\n", best.CL, best.A,
@@ -982,7 +1118,9 @@ ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want
     at[0].val.clusterDim.x = (unsigned)cfg.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     lc.gridDim = dim3((unsigned)(cfg.CL * cfg.n_clusters)); lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
     lc.dynamicSmemBytes = cfg.smem; lc.stream = q; lc.attrs = at; lc.numAttrs = 1;
-    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, want));
+    ts_fire_params nofire;
+    memset(&nofire, 0, sizeof nofire);
+    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, want, nofire));
     st->launches += 1;
     st->last_engine = 1;
     st->list_built = false;          /* the general engine's list no longer matches the positions */
@@ -1001,4 +1139,45 @@ extern "C" int ts_debug_resident_profile(unsigned long long *out16)
     (void)out16;
     return 2;
 #endif
+}
+
+/* FIRE relaxation inside the resident engine: the same kernel in FIRE mode (per-system dt, the four reductions and
+ * the state machine after every step, finished systems skipped bit-unchanged). */
+ts_status resident_fire(ts_state *st, const ts_fire_params &fp, int n_steps, cudaStream_t q)
+{
+    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
+    ResPlan *p = plan_of(st);
+    ResCfg cfg = p->cfg;
+    ResKernel k = pick_kernel(st, true);
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)cfg.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
+    lc.dynamicSmemBytes = cfg.smem; lc.stream = q; lc.attrs = at; lc.numAttrs = 1;
+    if (p->fire_clusters == 0) {                     /* the FIRE variant has its own register count and occupancy */
+        if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem) != cudaSuccess) {
+            cudaGetLastError();
+            return TS_ERR_UNSUPPORTED;
+        }
+        lc.gridDim = dim3((unsigned)(cfg.CL * st->d.S));
+        int maxc = 0;
+        if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
+            cudaGetLastError();
+            return TS_ERR_UNSUPPORTED;
+        }
+        p->fire_clusters = st->d.S < maxc ? st->d.S : maxc;
+    }
+    cfg.n_clusters = p->fire_clusters;
+    lc.gridDim = dim3((unsigned)(cfg.CL * cfg.n_clusters));
+    TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
+    MdConst c;
+    memset(&c, 0, sizeof c);
+    c.integrator = TS_NVE;
+    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, (unsigned)TS_WANT_ENERGY, fp));
+    st->launches += 1;
+    st->last_engine = 1;
+    st->list_built = false;          /* the general engine's list no longer matches the positions */
+    return TS_OK;
 }

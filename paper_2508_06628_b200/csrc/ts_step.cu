@@ -103,6 +103,13 @@ extern "C" ts_status ts_fire_step(ts_state *st, const ts_fire_params *p, int32_t
     NEED_STATE(st);
     if (!p || n_steps < 0 || !(p->dt_start > 0.0) || !(p->dt_max > 0.0) || !(p->f_max > 0.0)) return TS_ERR_INVALID_ARG;
     cudaStream_t q = (cudaStream_t)stream;
+    if (st->engine == 1 && resident_supported(st)) {
+        ts_status rc = resident_fire(st, *p, n_steps, q);
+        if (rc != TS_ERR_UNSUPPORTED) {
+            if (rc == TS_OK) { st->steps_done += n_steps; st->forces_current = true; }
+            return rc;
+        }
+    }
     st->last_engine = 0;
     launch_fire_init(st, *p, q);
     ensure_list(st, q);
