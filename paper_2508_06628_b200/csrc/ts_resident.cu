@@ -952,11 +952,12 @@ static ResKernel pick_kernel(const ts_state *st, bool fire = false)
 static unsigned up16(unsigned x) { return (x + 15u) & ~15u; }
 
 /* Shared-memory carve for cluster size CL; returns false when it does not fit. */
-static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types)
+static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types, int thread_div = 1)
 {
     size_t w = dtype == TS_F32 ? 4 : 8;
     int A = ((((nmax + CL - 1) / CL) + 3) / 4) * 4;
-    const int max_threads = dtype == TS_F32 ? RES_MAX_THREADS : RES_MAX_THREADS_F64;
+    int max_threads = (dtype == TS_F32 ? RES_MAX_THREADS : RES_MAX_THREADS_F64) / thread_div;
+    if (getenv("TS_RES_MAXT")) max_threads = atoi(getenv("TS_RES_MAXT"));
     if (A > max_threads) return false;
     int pitch = 32 * ((need_row + 31) / 32);                     /* whole trips of 32 entries */
     int ntasks = A / 4, maxw = max_threads / 32;
@@ -1063,6 +1064,23 @@ bool resident_supported(ts_state *st)
         if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
             cudaGetLastError();
             return false;
+        }
+        /* many more systems than clusters in flight, and the atoms of a CTA fit half the threads: a half-size block
+         * lets two CTAs share an SM (registers were the limit), which hides the barrier latencies of small systems */
+        if (S >= 2 * maxc && !getenv("TS_RES_MAXT")) {
+            ResCfg h;
+            memset(&h, 0, sizeof h);
+            if (res_layout(h, out.CL, nmax, need_row, ns, d.dtype, d.n_types, 2) && h.nwarps < out.nwarps) {
+                lc.blockDim = dim3((unsigned)(h.nwarps * 32));
+                lc.dynamicSmemBytes = h.smem;
+                int maxc2 = 0;
+                if (cudaOccupancyMaxActiveClusters(&maxc2, (const void *)k, &lc) == cudaSuccess && maxc2 >= (3 * maxc) / 2) {
+                    out = h;
+                    maxc = maxc2;
+                } else {
+                    cudaGetLastError();
+                }
+            }
         }
         maxc_out = maxc;
         const int live = S < maxc ? S : maxc;
