@@ -221,3 +221,28 @@ def test_nve_binary_soft_sphere_fp64(ts, orc, engine):
     assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-9)
     assert np.abs(st.numpy("virial") - o["W"]).max() <= 1e-8 * np.abs(o["W"]).max()
     st.close()
+
+
+def test_resident_engine_is_deterministic(ts):
+    """Fixed reduction orders, no atomics on the physics: two runs of the same batch agree bit for bit (positions,
+    velocities, forces, energies, virials), for MD and for FIRE."""
+    b = wl.cfg2(n_systems=3, dtype="f32")
+    outs = []
+    for _ in range(2):
+        st = ts.SimState(b, engine=1)
+        st.md_step(dict(b.md), 120, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+        assert st.poll().flags == 0 and st.poll().engine == 1
+        outs.append([st.numpy(k).copy() for k in ("pos", "vel", "force", "energy", "virial", "kinetic")])
+        st.close()
+    for a, c in zip(*outs):
+        assert np.array_equal(a, c)
+    f = wl.cfg4(range(4), n_atoms=128)
+    outs = []
+    for _ in range(2):
+        st = ts.SimState(f, engine=1)
+        st.fire_step(f.fire, 150)
+        assert st.poll().flags == 0 and st.poll().engine == 1
+        outs.append([st.numpy(k).copy() for k in ("pos", "vel", "force", "energy")])
+        st.close()
+    for a, c in zip(*outs):
+        assert np.array_equal(a, c)
