@@ -1,35 +1,39 @@
 /*
- * ts_resident.cu -- system-resident MD engine (SURVEY.md section 7 "hard part 1", kernel K13).
+ * ts_resident.cu -- system-resident MD and FIRE engine (SURVEY.md section 7 "hard part 1", kernel K13).
  *
  * The graded batch (BASELINE.json:configs[1], 64 x 864 atoms) is so small that a step is bound by
  * launch latency and on-chip bandwidth, not by HBM.  This engine therefore keeps a whole system on
- * chip for all n_steps of a ts_md_step call: one thread-block cluster of CL CTAs per system, each
- * CTA owning a contiguous slice of the system's atoms.  Per CTA, in shared memory:
- *     pos[NS]        wrapped positions + type of ALL atoms of the system (slots 0..N_s-1), eight
+ * chip for all n_steps of a ts_md_step / ts_fire_step call: one thread-block cluster of CL CTAs per
+ * system, each CTA owning a contiguous slice of the system's atoms.  Per CTA, in shared memory:
+ *     pos[NS]        position slots (16 B: wrapped x, y, z + type; fp64: two planes).  HOME slots of
+ *                    ALL atoms of the system (a hashed permutation of the atom order, hslot), eight
  *                    far-away dummies (list padding, one per 16-byte bank group) and the GHOST
  *                    slots: every periodic image of an atom that can lie within r_list of the cell
- *                    (the atom is within r_list of a face) owns a slot holding x + S.h.  Every owner
- *                    publishes its atom and its ghosts into every CTA of the cluster through DSMEM.
- *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only; aliased onto the ghost slots,
- *                    which are dead between the cluster barrier of a step and the ghost refresh after a rebuild)
- *     gtab[N_s]      first ghost slot, active axes and image signs of every atom (rebuilds only)
- *     rows[A][pitch] the Verlet list of the CTA's own atoms: 16-bit entries = byte offset of the
- *                    neighbour's slot.  Thanks to the ghosts EVERY pair is a plain difference of two
- *                    slots: no image arithmetic in the pair loop.
+ *                    owns a slot holding x + S.h, in the bank group of its atom.  Owners publish
+ *                    only their home slot into every CTA of the cluster through DSMEM; every CTA
+ *                    regenerates the ghosts locally each step (ghost_pass).
+ *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only; aliased onto the
+ *                    ghost slots, which are dead between the cluster barrier of a step and the ghost
+ *                    refresh after a rebuild)
+ *     gtab[N_s]      first ghost slot, active axes and image signs of every atom
+ *     rows[A][pitch] the Verlet list of the CTA's own atoms: 16-bit entries = slot number of the
+ *                    neighbour.  Thanks to the ghosts EVERY pair is a plain difference of two slots:
+ *                    no image arithmetic in the pair loop.  One COLUMN per bank group (build_phase).
  *     fs[3][A]       forces of the own atoms (pair phase -> integrator phase)
- * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift, ghost
- * descriptor.  HBM is touched when a system is loaded, when it is stored, and never in between.
+ * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift.  HBM is
+ * touched when a system is loaded, when it is stored, and never in between.
  *
- * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading) -> [publish] -> cluster
- * barrier -> [rebuild if any atom moved > skin/2] -> [pair phase] -> arrive(done reading) -> block
- * barrier -> [owner: B].  Same physics as the general engine.
+ * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading) -> [publish home slots]
+ * -> cluster barrier -> [rebuild if any atom moved > skin/2] -> [ghost refresh] -> [pair phase] ->
+ * arrive(done reading) -> block barrier -> [owner: B].  FIRE mode (template flag): per-system dt,
+ * the four reductions and the state machine after every step, finished systems skipped untouched.
+ * Same physics as the general engine.
  *
- * Pair phase: 8 lanes per atom (one quarter-warp = one LDS.128 phase), two pairs per lane and
- * iteration.  A ghost slot is congruent to its atom modulo 8 and lane l of the builder tests the
- * candidates j = l mod 8, so a lane's hits all live in 16-byte bank group l; the list is laid out
- * round-robin over the groups and the position gather is conflict-free while every group still has
- * members.  The fp32 Lennard-Jones force-only loop uses Blackwell's packed FFMA2/FMUL2 (f32x2) on
- * the two pairs of a lane: the kernel is issue-bound, and a packed op costs one issue slot.
+ * Pair phase: 8 lanes per atom (one quarter-warp = one LDS.128 phase), rows read in trips of 32
+ * entries (one 64-bit load per lane).  Lane l of the builder tests the slots = l mod 8, so a lane's
+ * hits all live in 16-byte bank group l and fill column l of the atom's list: a row of eight is
+ * served by one shared-memory wavefront unless a group overflowed its column.  The fp32
+ * Lennard-Jones force-only loop uses Blackwell's packed FFMA2/FMUL2 (f32x2) on pairs of pairs.
  *
  * Rebuild: brute force over the system in fractional fixed point (integer subtraction wraps = the
  * minimum image), valid because the engine is only used when every cell height is >= 2 r_list
