@@ -23,8 +23,10 @@
  * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift.  HBM is
  * touched when a system is loaded, when it is stored, and never in between.
  *
- * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading) -> [publish home slots]
- * -> cluster barrier -> [rebuild if any atom moved > skin/2] -> [ghost refresh] -> [pair phase] ->
+ * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading; split-phase cluster
+ * barrier, no fence) -> [publish home slots with st.async: they complete transaction bytes on the
+ * receiving CTA's mbarrier, the skin flag rides in the slot's type word] -> wait on the own mbarrier
+ * -> [ghost refresh] -> [rebuild if any atom moved > skin/2, then ghosts again] -> [pair phase] ->
  * arrive(done reading) -> block barrier -> [owner: B].  FIRE mode (template flag): per-system dt,
  * the four reductions and the state machine after every step, finished systems skipped untouched.
  * Same physics as the general engine.
@@ -67,7 +69,7 @@ struct ResCfg {
     int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
-    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc, o_fire;
+    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
     unsigned smem;
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
 };
@@ -94,22 +96,63 @@ __device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arri
 __device__ __forceinline__ void cl_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
+/* ------------------------------------------------------------------ mbarrier for the per-step position exchange
+ * Every CTA owns one FULL mbarrier.  The owners of the cluster send the home slots with st.async, which completes
+ * transaction bytes on the RECEIVING CTA's barrier; a CTA waits on its own barrier only: no cluster-wide barrier
+ * with a GPU-scope release fence (MEMBAR.ALL.GPU + CCTL.IVALL) on the critical path of a step.  The write-after-
+ * read side (peers have finished reading the old slots) stays on the split-phase cluster barrier, whose arrive
+ * needs no fence. */
+__device__ __forceinline__ void mb_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mb_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mb_wait(unsigned bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ unsigned map_cluster(unsigned saddr, unsigned rank)
+{
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_async_pos(unsigned dst, unsigned bar, unsigned, float x, float y, float z, int ty)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
+                 :: "r"(dst), "f"(x), "f"(y), "f"(z), "f"(__int_as_float(ty)), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void st_async_pos(unsigned dst, unsigned bar, unsigned zt, double x, double y, double z, int ty)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 :: "r"(dst), "d"(x), "d"(y), "r"(bar) : "memory");
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 :: "r"(dst + zt), "d"(z), "d"(__longlong_as_double((long long)ty)), "r"(bar) : "memory");
+}
+#define MOVED_BIT 0x40000000              /* in the type word of a home slot: its atom moved more than skin / 2 */
+
 /* ------------------------------------------------------------------ position slots */
 template <typename T> struct P3 { T x, y, z; int ty; };
 
 __device__ __forceinline__ P3<float> ld_pos(const unsigned char *base, unsigned off, unsigned, float)
 {
     float4 v = *(const float4 *)(base + off);
-    P3<float> p; p.x = v.x; p.y = v.y; p.z = v.z; p.ty = __float_as_int(v.w);
+    P3<float> p; p.x = v.x; p.y = v.y; p.z = v.z; p.ty = __float_as_int(v.w) & 0xff;        /* bit 30: MOVED_BIT */
     return p;
 }
 __device__ __forceinline__ P3<double> ld_pos(const unsigned char *base, unsigned off, unsigned zt, double)
 {
     double2 a = *(const double2 *)(base + off);
     double2 b = *(const double2 *)(base + zt + off);
-    P3<double> p; p.x = a.x; p.y = a.y; p.z = b.x; p.ty = (int)__double_as_longlong(b.y);
+    P3<double> p; p.x = a.x; p.y = a.y; p.z = b.x; p.ty = (int)__double_as_longlong(b.y) & 0xff;
     return p;
 }
+__device__ __forceinline__ int ld_tyword(const unsigned char *base, unsigned off, unsigned, float) { return *(const int *)(base + off + 12u); }
+__device__ __forceinline__ int ld_tyword(const unsigned char *base, unsigned off, unsigned zt, double) { return *(const int *)(base + zt + off + 8u); }
 __device__ __forceinline__ void st_pos(unsigned char *base, unsigned off, unsigned, float x, float y, float z, int ty)
 {
     *(float4 *)(base + off) = make_float4(x, y, z, __int_as_float(ty));
@@ -167,9 +210,11 @@ __device__ __forceinline__ void publish_home(cg::cluster_group &cluster, int CL,
 
 /* every CTA refreshes the images of every atom of the system from the home slots */
 template <typename T>
-__device__ __forceinline__ void ghost_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int N_s)
+__device__ __forceinline__ bool ghost_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int N_s)
 {
+    bool moved = false;                      /* MOVED_BIT of any home slot visited: the owner's skin check (R12) */
     for (int j = threadIdx.x; j < N_s; j += (int)blockDim.x) {
+        moved |= (ld_tyword(posb, (unsigned)j * 16u, zt, (T)0) & MOVED_BIT) != 0;
         const unsigned e = gtab[j];
         const unsigned act = (e >> 16) & 7u;
         if (act == 0u) continue;
@@ -196,6 +241,7 @@ __device__ __forceinline__ void ghost_pass(unsigned char *posb, unsigned zt, con
             }
         }
     }
+    return moved;
 }
 
 /* ------------------------------------------------------------------ one pair (generic path) */
@@ -668,6 +714,13 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     FireSm *fsm = (FireSm *)(smem + rc.o_fire);
     double *fred = (double *)(fsm + 1);   /* per-warp scratch of fire_reduce, [nwarps][8] */
 
+    const unsigned mb_full = smem_u32(smem + rc.o_mbar);
+    const unsigned pos_sa = smem_u32(posb);
+    unsigned full_parity = 0u;
+    if (tid == 0) {
+        mb_init(mb_full, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
 
@@ -741,7 +794,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         long long prof_acc[12] = { 0 }, prof_t = clock64();
 #endif
         for (int n = 0; n <= n_steps; ++n) {
-            const int nb = n & 1;
+            bool rebuild = n == 0;
             if (FIRE && n > 0) {
                 if (fsm->nsteps >= fp.max_steps) {     /* reported as failed, never counted (R24) */
                     __syncthreads();
@@ -776,20 +829,25 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 TICK(0);
                 if (!FIRE) cl_wait();                 /* every CTA of the cluster has finished reading the old positions (FIRE: fire_reduce's barriers) */
                 TICK(1);
+                if (tid == 0) mb_expect_tx(mb_full, (unsigned)N_s * (unsigned)(4 * sizeof(T)));   /* this step's home slots */
                 if (own) {
-                    if (moved)
-                        for (int r = 0; r < CL; ++r) cluster.map_shared_rank(misc, r)->flags[nb] = 1;
-                    publish_home<T>(cluster, CL, posb, zt, hs, x0 - ws0, x1 - ws1, x2 - ws2, ty);
+                    const T px = x0 - ws0, py = x1 - ws1, pz = x2 - ws2;
+                    const int tyw = ty | (moved ? MOVED_BIT : 0);         /* the skin flag travels with the slot */
+                    for (int r = 0; r < CL; ++r)
+                        st_async_pos(map_cluster(pos_sa + (unsigned)hs * 16u, (unsigned)r), map_cluster(mb_full, (unsigned)r), zt, px, py, pz, tyw);
                 }
                 TICK(2);
-                cl_arrive();
-                cl_wait();                            /* new positions (and the rebuild flag) visible everywhere */
+                mb_wait(mb_full, full_parity);        /* all home slots of the step have arrived in THIS CTA */
+                full_parity ^= 1u;
                 TICK(3);
+                /* images of the new home positions (local) and the owners' skin flags */
+                rebuild = __syncthreads_or(ghost_pass<T>(posb, zt, gtab, gh, N_s) ? 1 : 0) != 0;
             }
-            const bool rebuild = (n == 0) || (misc->flags[nb] != 0);
             if (rebuild) {
-                __syncthreads();
-                if (tid == 0) { misc->flags[nb] = 0; misc->rebuilds += 1u; misc->nnz = 0u; }
+                /* every CTA of the cluster takes this branch in the same step (the flags travel with the home slots);
+                 * nobody may still be reading its home / ghost slots when the re-wrapped slots and fr arrive */
+                cluster.sync();
+                if (tid == 0) { misc->rebuilds += 1u; misc->nnz = 0u; }
                 if (own) {
                     /* wrap into the cell: f = x . h^-1, w = floor(f) (R5: the stored x stays unwrapped) */
                     T fa = x0 * gh[9] + x1 * gh[12] + x2 * gh[15];
@@ -820,9 +878,9 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 build_phase(rc, fr, gtab, rows, cnt, G, G[6], a_begin, A_own, N_s, N8, misc);
                 __syncthreads();
                 TICK(7);
+                ghost_pass<T>(posb, zt, gtab, gh, N_s);          /* images again: the rebuild re-wrapped the home slots */
+                __syncthreads();
             }
-            ghost_pass<T>(posb, zt, gtab, gh, N_s);              /* images of the new home positions, local */
-            __syncthreads();
             TICK(10);
             const bool last = n == n_steps;
             if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
@@ -985,6 +1043,7 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.o_cred = o; o += 8u * 64u;
     c.o_misc = o; o += up16((unsigned)(sizeof(ResMisc) + 18 * w + 8 * sizeof(float) + 4 * sizeof(unsigned)));
     c.o_fire = o; o += up16((unsigned)(sizeof(FireSm) + (RES_MAX_THREADS / 32) * 64u));
+    c.o_mbar = o; o += 16u;                                       /* FULL mbarrier of the position exchange */
     c.smem = o;
     return o <= RES_SMEM_LIMIT;
 }
