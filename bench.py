@@ -28,7 +28,7 @@ sys.path.insert(0, ROOT)
 import workloads as wl  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_resident_md launch (1000 MD steps), profiles/r01_ncu_resident_cfg2_fp32.md
-NCU_TRAFFIC = {"resident": 1.897728e6 + 1280.0, "general": None}
+NCU_TRAFFIC = {"resident": 1.895936e6 + 1280.0, "general": None}
 
 METRIC = "atom_steps_per_s"
 UNIT = "atom-steps/s"
