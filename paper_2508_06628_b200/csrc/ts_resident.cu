@@ -75,7 +75,7 @@ struct ResCfg {
 };
 
 struct ResMisc {
-    int flags[2];
+    int unused[2];
     unsigned nnz;
     unsigned rebuilds;
     int overflow;
@@ -90,7 +90,6 @@ __device__ unsigned long long g_res_prof[16];
 #define TICK(k) do { } while (0)
 #endif
 
-__device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 /* "this CTA has finished READING the positions of the step": nothing was written, so no release fence is needed
  * (the loads completed before their values were consumed); the matching wait still acquires */
 __device__ __forceinline__ void cl_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
@@ -757,7 +756,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 double rho = (rb + 2.0 * (double)rc.eps_rel * lmax) / geo.hperp[k] + 1e-6;
                 thr[k] = rho >= 0.5 ? 0x80000000u : (unsigned)(rho * 4294967296.0);
             }
-            misc->flags[0] = 0; misc->flags[1] = 0; misc->nnz = 0u; misc->rebuilds = 0u; misc->overflow = 0;
+            misc->nnz = 0u; misc->rebuilds = 0u; misc->overflow = 0;
             if (FIRE) {
                 const bool fresh = fstat0 == TS_FIRE_FRESH;
                 fsm->dt = fresh ? fp.dt_start : d.f_dt[s];
