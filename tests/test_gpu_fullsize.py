@@ -162,3 +162,21 @@ def test_cfg5_liquid_fp32_large_batch(ts, orc):
     E1 = st.numpy("energy") + st.numpy("kinetic")
     assert np.abs(E1 - E0).max() <= 5e-3 * 1000              # NVE drift per system over 200 steps, reduced units
     st.close()
+
+
+def test_cfg2_long_run_thermostat_and_stability(ts):
+    """configs[1] for 20,000 BAOAB steps on the benched launch: no error flag, everything finite, and the kinetic
+    temperature of the batch sits at the thermostat's 80 K (per-system sigma_T = T sqrt(2 / 3N) = 2.2 K; the mean over 64
+    systems must be within 1.5 K, every system within 6 sigma)."""
+    b = wl.cfg2(n_systems=64, dtype="f32")
+    st = ts.SimState(b)
+    for _ in range(20):
+        st.md_step(dict(b.md), 1000)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 1 and rep.steps_done == 20000
+    assert np.isfinite(st.numpy("pos")).all() and np.isfinite(st.numpy("vel")).all()
+    T = 2.0 * st.numpy("kinetic") / (3 * 864 * b.kB)
+    assert abs(T.mean() - 80.0) < 1.5
+    assert np.all(np.abs(T - 80.0) < 6 * 2.2)
+    _net_force_is_zero(b, st, rel=1e-3)
+    st.close()
