@@ -43,6 +43,7 @@ TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types
     L.f_status = take(4 * (size_t)S);
     L.f_acc = take(8 * 4 * (size_t)S);
     L.sys_active = take(4 * (size_t)S);
+    L.sys_rebuild = take(4 * (size_t)S);
     L.sys_step = take(8 * (size_t)S);
     L.uid_own = take(4 * (size_t)S);
     L.scratch = take(4 * (2 * (size_t)S + 8));
@@ -234,7 +235,7 @@ extern "C" ts_status ts_state_create(const ts_state_desc *desc, const ts_potenti
     d.nbr_base = (long long *)(ws + L.nbr_base); d.nbr_len = (long long *)(ws + L.nbr_len);
     d.f_dt = (double *)(ws + L.f_dt); d.f_alpha = (double *)(ws + L.f_alpha);
     d.f_npos = (int *)(ws + L.f_npos); d.f_nsteps = (int *)(ws + L.f_nsteps); d.f_status = (int *)(ws + L.f_status);
-    d.f_acc = (double *)(ws + L.f_acc); d.sys_active = (int *)(ws + L.sys_active);
+    d.f_acc = (double *)(ws + L.f_acc); d.sys_active = (int *)(ws + L.sys_active); d.sys_rebuild = (int *)(ws + L.sys_rebuild);
     d.sys_step = (unsigned long long *)(ws + L.sys_step); d.uid_own = (unsigned int *)(ws + L.uid_own);
     d.scratch = (int *)(ws + L.scratch); d.pot = ws + L.pot;
     d.pos4 = ws + L.pos4; d.spos = (double4 *)(ws + L.spos); d.xref = ws + L.xref;

@@ -67,22 +67,30 @@ __global__ void k_geometry(DevState d, const int *slots, int count)
     for (int k = 0; k < 9; ++k) hT[k] = c[k];
 }
 
+/* Only the systems whose skin flag is set (sys_rebuild) are rebuilt: every system has its own bin range, its own
+ * CSR segment and its own reference positions, so a build touches nothing of the others (R12). */
 __global__ void k_build_begin(DevState d)
 {
     if (!d.status->need_rebuild) return;
-    long long n = d.N + d.S + 1;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
-        d.cell_count[i] = 0;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < d.S; i += (long long)gridDim.x * blockDim.x)
-        d.nbr_len[i] = 0;                     /* row cursor of the system's CSR segment (k_nbr_fill) */
+    for (int s = blockIdx.x; s < d.S; s += gridDim.x) {
+        if (!d.sys_rebuild[s]) continue;
+        const int base = ts_cell_base(d.sysoff, s), nc = d.geom[s].ncell;
+        for (int c = threadIdx.x; c <= nc; c += blockDim.x) d.cell_count[base + c] = 0;
+        if (threadIdx.x == 0) d.nbr_len[s] = 0;                /* row cursor of the system's CSR segment (k_nbr_fill) */
+    }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         d.status->nnz = 0ull;
-        d.status->max_nbr = 0u;
         d.status->list_valid = 1u;
+        d.status->n_rebuilds += 1;
     }
 }
 
-__global__ void k_build_end(DevState d) { d.status->need_rebuild = 0u; }
+__global__ void k_build_end(DevState d)
+{
+    /* no early exit here: block 0 clears need_rebuild, and a block that starts later must still clear its flags */
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < d.S; s += gridDim.x * blockDim.x) d.sys_rebuild[s] = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) d.status->need_rebuild = 0u;
+}
 
 template <typename T>
 __global__ void k_bin(DevState d)
@@ -91,6 +99,7 @@ __global__ void k_bin(DevState d)
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.N) return;
     int s = d.sysidx[i];
+    if (!d.sys_rebuild[s]) return;
     const SysGeom &g = d.geom[s];
     const T *x = (const T *)d.pos + 3 * i;
     double x0 = (double)x[0], x1 = (double)x[1], x2 = (double)x[2];
@@ -149,6 +158,7 @@ __global__ void k_cellscan(DevState d)
     if (!d.status->need_rebuild) return;
     __shared__ int sh[33];
     int s = blockIdx.x;
+    if (!d.sys_rebuild[s]) return;
     int base = ts_cell_base(d.sysoff, s);
     int nc = d.geom[s].ncell;
     int run = d.sysoff[s];
@@ -162,7 +172,6 @@ __global__ void k_cellscan(DevState d)
     }
     if (threadIdx.x == 0) {
         d.cell_start[base + nc] = run;
-        if (s == 0) d.status->n_rebuilds += 1;
     }
 }
 
@@ -173,6 +182,7 @@ __global__ void k_scatter(DevState d)
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.N) return;
     int s = d.sysidx[i];
+    if (!d.sys_rebuild[s]) return;
     const SysGeom &g = d.geom[s];
     const T *x = (const T *)d.pos + 3 * i;
     T xs0 = x[0], xs1 = x[1], xs2 = x[2];
@@ -217,12 +227,12 @@ __global__ void __launch_bounds__(256) k_nbr_fill(DevState d)
     const unsigned lt = (1u << l) - 1u;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
     const double R2 = d.r_list2;
-    unsigned long long nnz = 0ull;
     unsigned mx = 0u;
     for (long long p4 = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 4; p4 < d.N; p4 += nwarps * 4) {
         const long long p = p4 + qg;
         if (p >= d.N) continue;
         const int s = d.sysidx[p];           /* sorted slots of a system occupy the system's own range */
+        if (!d.sys_rebuild[s]) continue;
         const SysGeom &g = d.geom[s];
         const int a0 = d.sysoff[s];
         const int base = a0 + s;
@@ -281,20 +291,13 @@ __global__ void __launch_bounds__(256) k_nbr_fill(DevState d)
         if (l == 0) {
             d.nbr_off[a0 + li] = seg + start;
             d.nbr_cnt[a0 + li] = cnt;
-            nnz += (unsigned long long)cnt;
             mx = max(mx, (unsigned)cnt);
         }
     }
     /* statistics: one atomic per warp */
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        nnz += __shfl_xor_sync(0xffffffffu, nnz, o);
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    }
-    if (lane == 0 && nnz) {
-        atomicAdd(&d.status->nnz, nnz);
-        atomicMax(&d.status->max_nbr, mx);
-    }
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (lane == 0 && mx) atomicMax(&d.status->max_nbr, mx);
 }
 
 /* cursor -> state of the segment: pairs in use, or -1 when the rows did not fit (overflow: flagged, list invalid) */
@@ -304,11 +307,14 @@ __global__ void k_nbr_finish(DevState d)
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= d.S) return;
     const long long cap = d.nbr_base[s + 1] - d.nbr_base[s];
-    if (d.nbr_len[s] > cap) {
+    long long len = d.nbr_len[s];
+    if (d.sys_rebuild[s] && len > cap) {
+        len = -1;
         d.nbr_len[s] = -1;
         atomicOr(&d.status->flags, TS_FLAG_NBR_OVERFLOW);
-        d.status->list_valid = 0u;
     }
+    if (len < 0) d.status->list_valid = 0u;                    /* also a system that overflowed earlier and was not rebuilt */
+    else atomicAdd(&d.status->nnz, (unsigned long long)len);  /* pairs of the whole batch, rebuilt or not */
 }
 
 /* ------------------------------------------------------------------ host launchers */
@@ -323,26 +329,25 @@ void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, c
 
 __global__ void k_force_rebuild(DevState d)
 {
-    d.status->need_rebuild = 1u;
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < d.S; s += gridDim.x * blockDim.x) d.sys_rebuild[s] = 1;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { d.status->need_rebuild = 1u; d.status->max_nbr = 0u; }
 }
 
 void launch_build(ts_state *st, bool force, cudaStream_t q)
 {
     const DevState &d = st->d;
-    if (force) { k_force_rebuild<<<1, 1, 0, q>>>(d); st->launches += 1; }
-    long long n = d.N + d.S + 1;
+    if (force) { k_force_rebuild<<<(d.S + 255) / 256, 256, 0, q>>>(d); st->launches += 1; }
     int tb = 256;
-    int nbz = (int)((n + tb - 1) / tb); if (nbz > 148 * 8) nbz = 148 * 8;
     int nba = (int)((d.N + tb - 1) / tb);
     long long nwarp_blocks = (d.N * 8 + tb - 1) / tb;          /* 8 lanes per atom ... */
     if (nwarp_blocks > 148 * 16) nwarp_blocks = 148 * 16;       /* ... in a capped, grid-stride grid */
-    k_build_begin<<<nbz, tb, 0, q>>>(d);
+    k_build_begin<<<d.S < 148 * 8 ? d.S : 148 * 8, tb, 0, q>>>(d);
     if (d.dtype == TS_F32) k_bin<float><<<nba, tb, 0, q>>>(d); else k_bin<double><<<nba, tb, 0, q>>>(d);
     k_cellscan<<<d.S, 256, 0, q>>>(d);
     if (d.dtype == TS_F32) k_scatter<float><<<nba, tb, 0, q>>>(d); else k_scatter<double><<<nba, tb, 0, q>>>(d);
     k_nbr_fill<<<(unsigned)nwarp_blocks, tb, 0, q>>>(d);
     k_nbr_finish<<<(d.S + 255) / 256, 256, 0, q>>>(d);
-    k_build_end<<<1, 1, 0, q>>>(d);
+    k_build_end<<<(d.S + 255) / 256, 256, 0, q>>>(d);
     st->launches += 7;
     st->list_built = true;
 }

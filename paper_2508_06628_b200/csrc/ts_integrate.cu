@@ -25,7 +25,7 @@ __device__ __forceinline__ void publish_pos(const DevState &d, long long i, int 
     ((V4 *)d.pos4)[i] = q;
     const T *xr = (const T *)d.xref + 3 * i;
     T a = x0 - xr[0], b = x1 - xr[1], c = x2 - xr[2];
-    if ((double)(a * a + b * b + c * c) > d.half_skin2) d.status->need_rebuild = 1u;
+    if ((double)(a * a + b * b + c * c) > d.half_skin2) { d.status->need_rebuild = 1u; d.sys_rebuild[s] = 1; }   /* only this system is rebuilt (R12) */
 }
 
 template <typename T>

@@ -81,6 +81,7 @@ struct DevState {
     int *f_npos, *f_nsteps, *f_status;
     double *f_acc;               /* [S,4] fmax2, P, vv, ff             */
     int *sys_active;             /* [S] 1 = atoms of the system move   */
+    int *sys_rebuild;            /* [S] 1 = an atom of the system moved > skin/2: its list is rebuilt at the next build (R12) */
     unsigned long long *sys_step;/* [S] per-system step counter (R18)  */
     unsigned int *uid_own;       /* [S] persistent ids (copy or iota)  */
     /* workspace: per atom */
@@ -119,7 +120,7 @@ struct ts_state {
 struct TsLayout {
     size_t total;
     size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
-        sys_active, sys_step, uid_own, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        sys_active, sys_rebuild, sys_step, uid_own, pos4, spos, xref, cell_count, cell_start, atom_cell,
         atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
 };
 TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);
