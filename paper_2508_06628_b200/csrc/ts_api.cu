@@ -93,7 +93,7 @@ extern "C" ts_status ts_estimate_system_bytes(int64_t n_atoms, double volume, do
         return TS_ERR_INVALID_ARG;
     size_t w = dtype == TS_F32 ? 4 : 8;
     size_t boundary = (size_t)n_atoms * (3 * 3 * w + w + 4 + 4) + 9 * w + 8 * 11 + 4;
-    size_t per_sys = sizeof(SysGeom) + 9 * w + 8 * 2 + 8 * 2 + 4 * 4 + 32 + 8 + 4 + 8 + 4 * 2 /* cell slots */;
+    size_t per_sys = sizeof(SysGeom) + 9 * w + 8 * 2 + 8 * 2 + 4 * 5 /* incl. sys_rebuild */ + 32 + 8 + 4 + 8 + 4 * 2 /* cell slots */;
     size_t ws = (size_t)n_atoms * per_atom_workspace_bytes(dtype) + per_sys +
                 4 * (size_t)system_pair_capacity(n_atoms, volume, r_list, slack);
     *out_bytes = boundary + ws;
