@@ -22,7 +22,11 @@
  * Pins (tests/test_oracle_*.py): closed-form dimers, FCC shell sums, F = -dE/dx and
  * W = -dE/dstrain by finite differences, Newton's third law, supercell / re-basis invariance,
  * brute-force pair enumeration over a fixed image cube, Philox known-answer vectors, NVE
- * reversibility + 2nd-order convergence + drift bound, BAOAB limits, FIRE on a harmonic dimer.
+ * reversibility + 2nd-order convergence + drift bounds (cfg1, cfg3), BAOAB limits and the Boltzmann
+ * bond fluctuation of a Morse dimer, FIRE on a harmonic dimer, the FIRE velocity mixing on a
+ * non-collinear cluster with the pre-update alpha (R21) and the P == 0 boundary, and Eabs against a
+ * dimer and an independent lattice sum with V of both signs (tests/test_oracle_pins_r2.py).
+ * No function of this file is "parity unpinned".
  */
 #include <math.h>
 #include <pthread.h>
