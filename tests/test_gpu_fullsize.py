@@ -25,7 +25,7 @@ def _sys_slice(b, s):
     return slice(int(b.sys_offset[s]), int(b.sys_offset[s + 1]))
 
 
-def _replay_check(ts, orc, b, st, samples, fp32=True, e_tol=2e-5):
+def _replay_check(ts, orc, b, st, samples, fp32=True, e_tol=1e-5):
     """R29 on sampled systems: the GPU's own positions go to the oracle; forces within 1e-4 max|F| (fp32) except
     atoms in a pair within 1e-5 of r_c (counted); energies within e_tol of max(|E|, sum 1/2 |V|)."""
     pos = st.numpy("pos").astype(np.float64)

@@ -180,7 +180,7 @@ def test_fp32_replay_parity_after_md(ts, orc, engine):
         fmax = np.linalg.norm(o["F"][a0:a1], axis=1).max()
         assert np.abs(F[a0:a1] - o["F"][a0:a1])[ok].max() <= 1e-4 * fmax
     scale = np.maximum(np.abs(o["E"]), o["Eabs"])
-    assert np.all(np.abs(st.numpy("energy") - o["E"]) <= 2e-5 * scale)
+    assert np.all(np.abs(st.numpy("energy") - o["E"]) <= 1e-5 * scale)
     st.close()
 
 
