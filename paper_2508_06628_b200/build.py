@@ -17,6 +17,8 @@ SOURCES = ["ts_api.cu", "ts_step.cu", "ts_build.cu", "ts_pair.cu", "ts_integrate
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+if os.environ.get("TS_DBG"):
+    FLAGS.append("-D" + os.environ["TS_DBG"])
 if os.environ.get("TS_RES_TIMING"):      # debugging aid: per-phase cycle counters in the resident kernel
     FLAGS.append("-DTS_RES_TIMING")
 

@@ -55,6 +55,22 @@
 #include "ts_rng.cuh"
 
 namespace cg = cooperative_groups;
+#ifdef DBG_MARK
+__device__ volatile int *g_dbg;
+__device__ __forceinline__ unsigned dbg_chk(unsigned a, unsigned fallback, int code, unsigned x0, unsigned x1)
+{
+    if (a >= 136000u || (a & 15u)) {
+        if (g_dbg) { int k = 64 + 8 * (int)(blockIdx.x & 3); if (g_dbg[k] == 0) { g_dbg[k] = code; g_dbg[k + 1] = (int)a; g_dbg[k + 2] = (int)x0; g_dbg[k + 3] = (int)x1; g_dbg[k + 4] = threadIdx.x; } }
+        return fallback;
+    }
+    return a;
+}
+#define CHK(a, fb, code, x0, x1) dbg_chk(a, fb, code, x0, x1)
+#define WMARK(code) do { if (g_dbg && (threadIdx.x & 31) == 0) { g_dbg[128 + 32 * (blockIdx.x & 3) + (threadIdx.x >> 5)] = (code); __threadfence_system(); } } while (0)
+#else
+#define WMARK(code) do { } while (0)
+#define CHK(a, fb, code, x0, x1) (a)
+#endif
 
 #define RES_MAX_THREADS 896         /* fp32; the fp64 kernels need twice the registers: 512 */
 #define RES_MAX_THREADS_F64 512
@@ -69,7 +85,7 @@ struct ResCfg {
     int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
-    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_cnt, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
+    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_meta, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
     unsigned smem;
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
 };
@@ -169,16 +185,6 @@ template <typename T> __device__ __forceinline__ T t_floor(T x);
 template <> __device__ __forceinline__ float t_floor<float>(float x) { return floorf(x); }
 template <> __device__ __forceinline__ double t_floor<double>(double x) { return floor(x); }
 
-/* u16 index of list slot p (p = 8 k + lane) inside a row: the four k of a trip are contiguous per lane */
-/* When the pitch is a multiple of 64 entries (rows 0 modulo 128 bytes apart) the odd rows store their
- * trips pairwise swapped (sw = 1), so that the 64-bit row loads of the two quarter-warps that share a
- * shared-memory phase never hit the same banks. */
-__device__ __forceinline__ int row_index(int p, int sw)
-{
-    int k = p >> 3, l = p & 7;
-    return (((k >> 2) ^ sw) << 5) + (l << 2) + (k & 3);
-}
-
 /* Home slot of atom j.  The bank group of a slot is slot mod 8; atoms that follow each other in a
  * regular pattern (a lattice written cell by cell) would load the groups of a neighbour list very
  * unevenly, so every block of eight atoms is rotated by a hash of the block number.  The last block
@@ -207,38 +213,62 @@ __device__ __forceinline__ void publish_home(cg::cluster_group &cluster, int CL,
     for (int r = 0; r < CL; ++r) st_pos(cluster.map_shared_rank(posb, r), (unsigned)ai * 16u, zt, px, py, pz, ty);
 }
 
-/* every CTA refreshes the images of every atom of the system from the home slots */
+/* the images of one atom: gtab entry e, home position (px, py, pz); image number r lives in slot base + 8 r */
 template <typename T>
-__device__ __forceinline__ bool ghost_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int N_s)
+__device__ __forceinline__ void ghost_write(unsigned char *posb, unsigned zt, unsigned e, const T *gh, T px, T py, T pz, int ty)
 {
-    bool moved = false;                      /* MOVED_BIT of any home slot visited: the owner's skin check (R12) */
+    const unsigned act = (e >> 16) & 7u;
+    if (act == 0u) return;
+    T a[3][3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const T sgn = ((e >> (19 + k)) & 1u) ? (T)1 : (T)-1;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) a[k][b] = sgn * gh[3 * k + b];
+    }
+    /* q[m] = p + sum_{k in m} a_k, built incrementally: q[m] = q[m without its top axis] + a_top */
+    T q[8][3] = { { px, py, pz } };
+    unsigned off = (e & 0xffffu) * 16u;
+#pragma unroll
+    for (int m = 1; m < 8; ++m) {
+        const int top = m >= 4 ? 2 : (m >= 2 ? 1 : 0);
+        const int rest = m & ~(1 << top);
+#pragma unroll
+        for (int b = 0; b < 3; ++b) q[m][b] = q[rest][b] + a[top][b];
+        if ((m & ~act) == 0u) {
+            st_pos(posb, off, zt, q[m][0], q[m][1], q[m][2], ty);
+            off += 128u;
+        }
+    }
+}
+
+/* every CTA refreshes the images of every atom of the system from the home slots (after a rebuild) */
+template <typename T>
+__device__ __forceinline__ void ghost_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int N_s)
+{
     for (int j = threadIdx.x; j < N_s; j += (int)blockDim.x) {
-        moved |= (ld_tyword(posb, (unsigned)j * 16u, zt, (T)0) & MOVED_BIT) != 0;
         const unsigned e = gtab[j];
-        const unsigned act = (e >> 16) & 7u;
-        if (act == 0u) continue;
+        if (((e >> 16) & 7u) == 0u) continue;
         const P3<T> p = ld_pos(posb, (unsigned)j * 16u, zt, (T)0);
-        T a[3][3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const T sgn = ((e >> (19 + k)) & 1u) ? (T)1 : (T)-1;
-#pragma unroll
-            for (int b = 0; b < 3; ++b) a[k][b] = sgn * gh[3 * k + b];
-        }
-        /* q[m] = p + sum_{k in m} a_k, built incrementally: q[m] = q[m without its top axis] + a_top */
-        T q[8][3] = { { p.x, p.y, p.z } };
-        unsigned off = (e & 0xffffu) * 16u;
-#pragma unroll
-        for (int m = 1; m < 8; ++m) {
-            const int top = m >= 4 ? 2 : (m >= 2 ? 1 : 0);
-            const int rest = m & ~(1 << top);
-#pragma unroll
-            for (int b = 0; b < 3; ++b) q[m][b] = q[rest][b] + a[top][b];
-            if ((m & ~act) == 0u) {
-                st_pos(posb, off, zt, q[m][0], q[m][1], q[m][2], p.ty);
-                off += 128u;
-            }
-        }
+        ghost_write<T>(posb, zt, e, gh, p.x, p.y, p.z, p.ty);
+    }
+}
+
+/* the new home positions of the other CTAs' atoms have arrived in the slot array (st.async): refresh their images and
+ * collect the owners' skin flags (R12), which travel in the type word.  [sb0, sb0 + sbw) are the CTA's own slots. */
+template <typename T>
+__device__ __forceinline__ bool peer_pass(unsigned char *posb, unsigned zt, const unsigned *gtab, const T *gh, int sb0, int sbw,
+                                          int n_peer_slots, int N_s)
+{
+    bool moved = false;
+    for (int k = threadIdx.x; k < n_peer_slots; k += (int)blockDim.x) {
+        const int hs = k < sb0 ? k : k + sbw;
+        if (hs >= N_s) continue;                 /* the unused slots of the last block */
+        moved |= (ld_tyword(posb, (unsigned)hs * 16u, zt, (T)0) & MOVED_BIT) != 0;
+        const unsigned e = gtab[hs];
+        if (((e >> 16) & 7u) == 0u) continue;
+        const P3<T> p = ld_pos(posb, (unsigned)hs * 16u, zt, (T)0);
+        ghost_write<T>(posb, zt, e, gh, p.x, p.y, p.z, p.ty);
     }
     return moved;
 }
@@ -291,7 +321,11 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
     return d;
 }
 
-/* ------------------------------------------------------------------ shared-space addressing */
+/* ------------------------------------------------------------------ shared-space addressing
+ * Addresses are shared-window addresses of THIS CTA (cvta: they carry the CTA's rank inside its cluster in bits 24+;
+ * an address without it is illegal on every CTA but rank 0).  The loads are volatile so that the gathers of the next
+ * trip stay ahead of the arithmetic of the current one. */
+extern __shared__ __align__(16) unsigned char ts_smem[];
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ float4 lds128(unsigned a)
 {
@@ -299,11 +333,26 @@ __device__ __forceinline__ float4 lds128(unsigned a)
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
     return v;
 }
-__device__ __forceinline__ uint2 lds64(unsigned a)
+__device__ __forceinline__ unsigned lds32(unsigned a)
 {
-    uint2 v;
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
+}
+/* position slot at shared-space address a (fp64: second plane zt bytes further) */
+__device__ __forceinline__ P3<float> ld_pos_sa(unsigned a, unsigned, float)
+{
+    const float4 v = lds128(a);
+    P3<float> p; p.x = v.x; p.y = v.y; p.z = v.z; p.ty = __float_as_int(v.w) & 0xff;
+    return p;
+}
+__device__ __forceinline__ P3<double> ld_pos_sa(unsigned a, unsigned zt, double)
+{
+    double2 u, w;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(u.x), "=d"(u.y) : "r"(a));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(w.x), "=d"(w.y) : "r"(a + zt));
+    P3<double> p; p.x = u.x; p.y = u.y; p.z = w.x; p.ty = (int)__double_as_longlong(w.y) & 0xff;
+    return p;
 }
 
 /* one packed step of the fp32 Lennard-Jones force loop: the two pairs (xi, pa) and (xi, pb) */
@@ -330,94 +379,115 @@ __device__ __forceinline__ void lj_pair2(const float4 &pa, const float4 &pb, flo
     FZ = fma2(G, RZ, FZ);
 }
 
-/* Forces of the CTA's own atoms from the shared-memory list; E and W partials into red (fp64).
- * A row is read in TRIPS of 32 entries: lane l of the atom's quarter-warp loads its four entries of
- * the trip with one 64-bit load (row_index).  FAST = fp32 Lennard-Jones, one type, forces only: the
- * pairs of a lane share packed ops two by two. */
-template <typename T, int KIND, bool NT1, bool EV>
-__device__ __forceinline__ void pair_phase(const ResCfg &rc, const unsigned char *posb, const unsigned short *rows,
-                                           const unsigned *cnt, const PotEntry<T> *tab, T *fs, int a_begin, int A_own,
-                                           int N8, int NT, double *red)
+/* ------------------------------------------------------------------ list layout
+ * The list of the four atoms of a task (one warp: quarter-warp q = atom, lane l = column = 16-byte bank group) is a
+ * sequence of TRIPS of 128 bytes: lane (q, l) owns the 32-bit word at q * 32 + l * 4, which holds two entries (list
+ * rows 2 t and 2 t + 1 of column l).  An entry is the number of a position slot (14 bits): the even row sits in bits
+ * 0..13, the odd row in bits 18..31, bits 14..17 are zero, so that the shared-memory address of the odd slot is one
+ * instruction (base + (word >> 14): LEA.HI) and the even one two (mask; base + 16 x: IMAD).  tmeta[4 task + q] =
+ * home slot of the atom | trips << 14 (the trip count is the same for the four atoms of a task). */
+#define ENT_MASK 0x3fffu
+__device__ __forceinline__ unsigned ent_even(unsigned w, unsigned base)
 {
+    unsigned a;
+    asm("mad.lo.u32 %0, %1, 16, %2;" : "=r"(a) : "r"(w & ENT_MASK), "r"(base));
+    return a;
+}
+__device__ __forceinline__ unsigned ent_odd(unsigned w, unsigned base) { return base + (w >> 14); }
+
+/* sum over the eight lanes of an atom of three values in four shuffles: lanes 0-1 end with fx, 2-3 fy, 4-5 fz */
+template <typename T>
+__device__ __forceinline__ T reduce3_8(T fx, T fy, T fz, int l)
+{
+    const bool h4 = (l & 4) != 0, h2 = (l & 2) != 0;
+    const T r0 = __shfl_xor_sync(0xffffffffu, h4 ? fx : fz, 4);
+    const T r1 = __shfl_xor_sync(0xffffffffu, fy, 4);
+    T a = (h4 ? fz : fx) + r0;                    /* lanes 0-3: fx of lanes {l, l ^ 4}; lanes 4-7: fz */
+    T b = h4 ? (T)0 : fy + r1;                    /* lanes 0-3: fy */
+    const T r2 = __shfl_xor_sync(0xffffffffu, h2 ? a : b, 2);
+    T v = (h2 ? b : a) + r2;                      /* lanes 0,1: fx; 2,3: fy; 4,5: fz; 6,7: 0 */
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
+}
+
+/* Forces of the CTA's own atoms from the shared-memory list; EV: energy and virial partials accumulate in fp64 (R31)
+ * and end as warp partials in red.  FAST = fp32 Lennard-Jones, one type, forces only: the two entries of a word
+ * share packed f32x2 operations, and the positions of trip t + 1 are gathered while trip t is computed. */
+template <typename T, int KIND, bool NT1, bool EV>
+__device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, unsigned rows_sa, const unsigned *tmeta,
+                                           const PotEntry<T> *tab, T *fs, int A_own, int NT, double *red)
+{
+    double acc[EV ? 7 : 1];
+    if (EV)
+#pragma unroll
+        for (int k = 0; k < 7; ++k) acc[k] = 0.0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
     const unsigned zt = (unsigned)rc.NS * 16u;
     const int ntasks = (A_own + 3) >> 2;
     constexpr bool FAST = (sizeof(T) == 4) && KIND == TS_LJ && NT1 && !EV;
-    const unsigned pos_sa = smem_u32(posb);
-    const unsigned row_sa0 = smem_u32(rows) + (unsigned)q * (unsigned)rc.pitch * 2u + (unsigned)l * 8u;
-    const unsigned task_stride = 4u * (unsigned)rc.pitch * 2u;
-    const unsigned sw = (rc.pitch & 63) == 0 ? (unsigned)(q & 1) : 0u;
-    double acc8[EV ? 7 : 1];
-    if (EV)
-#pragma unroll
-        for (int k = 0; k < 7; ++k) acc8[k] = 0.0;
+    const unsigned task_stride = (unsigned)rc.pitch * 8u;
+    const unsigned lane_off = (unsigned)q * 32u + (unsigned)l * 4u;
+    const PotEntry<T> pe1 = tab[0];
+    const float rc2f = (float)pe1.rc2, m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
-        T ev[7] = { 0, 0, 0, 0, 0, 0, 0 };
+        const unsigned meta = tmeta[task * 4 + q];
+        const int nt = (int)(meta >> 14);
+        const unsigned xa = pos_sa + ((meta & ENT_MASK) << 4);
         const int al = task * 4 + q;
         const bool has = al < A_own;
-        const int ai = hslot(a_begin + (has ? al : 0), N8);     /* home slot of the atom */
-        const int ntrip = (int)cnt[task];                       /* the same for the four atoms of a task */
-        const unsigned ra = row_sa0 + (unsigned)task * task_stride;
+        const unsigned ra = rows_sa + (unsigned)task * task_stride + lane_off;
         T fx = 0, fy = 0, fz = 0;
+        T ev[7] = { 0, 0, 0, 0, 0, 0, 0 };
         if (FAST) {
-            const float4 xi4 = lds128(pos_sa + (unsigned)ai * 16u);
-            const PotEntry<T> pe1 = tab[0];
-            const float xix = xi4.x, xiy = xi4.y, xiz = xi4.z, rc2 = (float)pe1.rc2;
-            const float m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
+            const float4 xi4 = lds128(xa);
+            const float xix = xi4.x, xiy = xi4.y, xiz = xi4.z;
             const f32x2 C12 = pk2(m12, m12), C6 = pk2(p6, p6);
             f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
-            uint2 e = lds64(ra + (sw << 6));
-            for (int t = 0; t < ntrip; ++t) {
-                const float4 p0 = lds128(pos_sa + ((e.x & 0xffffu) << 4));
-                const float4 p1 = lds128(pos_sa + ((e.x >> 16) << 4));
-                const float4 p2 = lds128(pos_sa + ((e.y & 0xffffu) << 4));
-                const float4 p3 = lds128(pos_sa + ((e.y >> 16) << 4));
-                e = lds64(ra + (((unsigned)(t + 1) ^ sw) << 6));      /* next trip's entries (one past the end is still inside smem) */
-                lj_pair2(p0, p1, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
-                lj_pair2(p2, p3, xix, xiy, xiz, rc2, C12, C6, FX, FY, FZ);
+            if (nt > 0) {
+                unsigned w = lds32(ra);
+                float4 p0 = lds128(ent_even(w, pos_sa)), p1 = lds128(ent_odd(w, pos_sa));
+                w = lds32(ra + 128u);                                    /* one word past the list is still inside shared memory */
+                for (int t = 1; t < nt; ++t) {
+                    const float4 q0 = lds128(ent_even(w, pos_sa)), q1 = lds128(ent_odd(w, pos_sa));
+                    w = lds32(ra + (unsigned)(t + 1) * 128u);
+                    lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
+                    p0 = q0; p1 = q1;
+                }
+                lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
             }
             float a, b;
             upk2(FX, a, b); fx = (T)(a + b);
             upk2(FY, a, b); fy = (T)(a + b);
             upk2(FZ, a, b); fz = (T)(a + b);
         } else {
-            const P3<T> xi = ld_pos(posb, (unsigned)ai * 16u, zt, (T)0);
-            const PotEntry<T> pe1 = tab[NT1 ? 0 : xi.ty * NT];
+            const P3<T> xi = ld_pos_sa(xa, zt, (T)0);
+            const PotEntry<T> pei = NT1 ? pe1 : tab[xi.ty * NT];
             const int tirow = xi.ty * NT;
-            for (int t = 0; t < ntrip; ++t) {
-                const uint2 e = lds64(ra + (((unsigned)t ^ sw) << 6));
-                const P3<T> x0 = ld_pos(posb, (e.x & 0xffffu) << 4, zt, (T)0);
-                const P3<T> x1 = ld_pos(posb, (e.x >> 16) << 4, zt, (T)0);
-                const P3<T> x2 = ld_pos(posb, (e.y & 0xffffu) << 4, zt, (T)0);
-                const P3<T> x3 = ld_pos(posb, (e.y >> 16) << 4, zt, (T)0);
-                pair_accum<T, KIND, NT1, EV>(xi, x0, pe1, tab, tirow, fx, fy, fz, ev);
-                pair_accum<T, KIND, NT1, EV>(xi, x1, pe1, tab, tirow, fx, fy, fz, ev);
-                pair_accum<T, KIND, NT1, EV>(xi, x2, pe1, tab, tirow, fx, fy, fz, ev);
-                pair_accum<T, KIND, NT1, EV>(xi, x3, pe1, tab, tirow, fx, fy, fz, ev);
+            unsigned w = lds32(ra);
+            for (int t = 0; t < nt; ++t) {
+                const P3<T> x0 = ld_pos_sa(ent_even(w, pos_sa), zt, (T)0);
+                const P3<T> x1 = ld_pos_sa(ent_odd(w, pos_sa), zt, (T)0);
+                w = lds32(ra + (unsigned)(t + 1) * 128u);
+                pair_accum<T, KIND, NT1, EV>(xi, x0, pei, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x1, pei, tab, tirow, fx, fy, fz, ev);
             }
         }
+        const T v = reduce3_8<T>(fx, fy, fz, l);
+        if (has && l < 6 && !(l & 1)) fs[(l >> 1) * rc.A + al] = v;
+        if (EV && has) {                /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
+            acc[0] += 0.5 * (double)ev[0];
 #pragma unroll
-        for (int o = 1; o < 8; o <<= 1) {
-            fx += __shfl_xor_sync(0xffffffffu, fx, o);
-            fy += __shfl_xor_sync(0xffffffffu, fy, o);
-            fz += __shfl_xor_sync(0xffffffffu, fz, o);
-        }
-        if (has && l < 3) fs[l * rc.A + al] = l == 0 ? fx : (l == 1 ? fy : fz);
-        if (EV) {                       /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
-            if (has) {
-                acc8[0] += 0.5 * (double)ev[0];
-#pragma unroll
-                for (int k = 1; k < 7; ++k) acc8[k] += -0.5 * (double)ev[k];
-            }
+            for (int k = 1; k < 7; ++k) acc[k] += -0.5 * (double)ev[k];
         }
     }
     if (EV) {                           /* warp partials of E, W into red[warp][0..6] */
 #pragma unroll
         for (int k = 0; k < 7; ++k) {
+            double a = acc[k];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc8[k] += __shfl_xor_sync(0xffffffffu, acc8[k], o);
-            if (lane == 0) red[warp * 8 + k] = acc8[k];
+            for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+            if (lane == 0) red[warp * 8 + k] = a;
         }
     }
 }
@@ -481,7 +551,7 @@ __device__ __forceinline__ unsigned wrap_bit(unsigned uj, unsigned ui)
 }
 
 __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, const unsigned *gtab, unsigned short *rows,
-                                            unsigned *cnt, const float *G, float rb2, int a_begin, int A_own, int N_s,
+                                            unsigned *tmeta, const float *G, float rb2, int a_begin, int A_own, int N_s,
                                             int N8, ResMisc *misc)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -546,24 +616,26 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
         int cq[8];                                                    /* populations of the eight bank groups of the atom */
 #pragma unroll
         for (int c = 0; c < 8; ++c) cq[c] = __shfl_sync(0xffffffffu, mine, c, 8);
-        int niter = (NT + 31) >> 5;                                 /* trips: u64 per lane, 32 entries per trip */
-        niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 8));
-        niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16)); /* the four atoms of a task share the loop count */
-        const bool fits = 32 * niter <= rc.pitch && !ovf;
+        int R = ((NT + 15) >> 4) << 1;                                /* rows: whole trips of 16 entries */
+        R = max(R, __shfl_xor_sync(0xffffffffu, R, 8));
+        R = max(R, __shfl_xor_sync(0xffffffffu, R, 16));              /* the four atoms of a task share the loop counts */
+        const bool fits = 8 * R <= rc.pitch && !ovf;
         if (!fits) {
             if (lane == 0) misc->overflow = 1;
-            niter = 0;
+            R = 0;
         }
-        unsigned short *row = rows + (size_t)al * rc.pitch;
-        const int sw = (rc.pitch & 63) == 0 ? (q & 1) : 0;
-        if (fits && niter > 0) {
-            /* Placement.  The pair loop reads R = 4 niter rows of eight entries; entry (row, column) is read by
-             * lane `column`, and one shared-memory wavefront serves a row when its eight bank groups differ.
-             * Lane l holds the hits of bank group l: its first R hits fill column l from the top (column = bank
-             * group, so those never collide), the rest of the column is padded with the far-away dummy of group
-             * l.  A group with more than R hits overflows: those hits take the free cells of the other columns in
+        /* u16 halves of the trip words of this atom: row r of column c lives at base + (r / 2) * 64 + c * 2 + (r & 1);
+         * the odd half holds the entry << 2 (bits 18..31 of the word) */
+        unsigned short *rowB = rows + (size_t)task * rc.pitch * 4 + q * 16;
+#define CELL_B(r, c) rowB[((r) >> 1) * 64 + (c) * 2 + ((r) & 1)]
+#define ENT(slot, r) (unsigned short)((unsigned)(slot) << (((r) & 1) << 1))
+        if (fits) {
+            /* Placement.  The pair loop reads R rows of eight entries; entry (row, column) is read by lane
+             * `column`, and one shared-memory wavefront serves a row when its eight bank groups differ.  Lane l
+             * holds the hits of bank group l: its first R hits fill column l from the top (column = bank
+             * group, so those never collide), the rest of the column is padded with the far-away dummy of group l.
+             * A group with more than R hits overflows: those hits take the free cells of the other columns in
              * column-major order, where they collide with their own group's column once each -- the minimum. */
-            const int R = 4 * niter;
             const int o_l = max(0, mine - R), f_l = max(0, R - mine);
             int io = o_l, jf = f_l;
 #pragma unroll
@@ -609,17 +681,20 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
                         prow = cc + (u - Fc);
                         ++u;
                     }
-                    row[row_index(8 * prow + pcol, sw)] = (unsigned short)slot;
+                    CELL_B(prow, pcol) = ENT(slot, prow);
                     ++m;
                 }
             }
             /* padding of my column below my own hits and the overflow entries it received */
-            for (int r = min(mine, R) + recv; r < R; ++r) row[row_index(8 * r + l, sw)] = (unsigned short)(N8 + l);
+            for (int r = min(mine, R) + recv; r < R; ++r) CELL_B(r, l) = ENT(N8 + l, r);
         }
-        if (lane == 0) cnt[task] = (unsigned)niter;
-        if (has && l == 0) nnz += (unsigned)NT;
+#undef CELL_B
+#undef ENT
+        if (l == 0) tmeta[task * 4 + q] = (unsigned)(has ? ai : N8) | ((unsigned)(R >> 1) << 14);
+        if (has) nnz += (unsigned)mine;
     }
-    if (nnz) atomicAdd(&misc->nnz, nnz);
+    nnz = __reduce_add_sync(0xffffffffu, nnz);
+    if (lane == 0 && nnz) atomicAdd(&misc->nnz, nnz);
 }
 
 /* ------------------------------------------------------------------ block / cluster reduction of 8 doubles */
@@ -685,24 +760,31 @@ __device__ __forceinline__ void fire_reduce(cg::cluster_group &cluster, int CL, 
     if (CL > 1) cluster.sync(); else __syncthreads();          /* cred may be rewritten by the next reduction */
 }
 
+#ifdef DBG_MARK
+extern "C" int ts_debug_set_marker(int *p) { return (int)cudaMemcpyToSymbol(g_dbg, &p, sizeof p); }
+#define MARK(k) do { __syncthreads(); if (g_dbg && threadIdx.x == 0) { g_dbg[blockIdx.x] = (k); __threadfence_system(); } } while (0)
+#else
+#define MARK(k) do { } while (0)
+#endif
 /* ------------------------------------------------------------------ the kernel */
 template <typename T, int KIND, bool NT1, bool FIRE>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THREADS_F64, 1) k_resident_md(DevState d, MdConst c, ResCfg rc, int n_steps, unsigned want, ts_fire_params fp)
 {
-    extern __shared__ __align__(16) unsigned char smem[];
+    unsigned char *const smem = ts_smem;
     cg::cluster_group cluster = cg::this_cluster();
     const int CL = rc.CL;
     const int rank = (int)cluster.block_rank();
     const int cid = (int)(blockIdx.x / (unsigned)CL);
     const int tid = threadIdx.x;
     const unsigned zt = (unsigned)rc.NS * 16u;
+    constexpr unsigned SB = 4u * (unsigned)sizeof(T);          /* bytes of a home slot */
 
     unsigned char *const posb = smem + rc.o_pos;
     uint4 *fr = (uint4 *)(smem + rc.o_fr);
     unsigned *gtab = (unsigned *)(smem + rc.o_gtab);
     unsigned short *rows = (unsigned short *)(smem + rc.o_rows);
     T *fs = (T *)(smem + rc.o_fs);
-    unsigned *cnt = (unsigned *)(smem + rc.o_cnt);
+    unsigned *tmeta = (unsigned *)(smem + rc.o_meta);
     PotEntry<T> *tab = (PotEntry<T> *)(smem + rc.o_pot);
     double *red = (double *)(smem + rc.o_red);
     double *cred = (double *)(smem + rc.o_cred);
@@ -715,6 +797,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
 
     const unsigned mb_full = smem_u32(smem + rc.o_mbar);
     const unsigned pos_sa = smem_u32(posb);
+    const unsigned rows_sa = smem_u32(rows);
     unsigned full_parity = 0u;
     if (tid == 0) {
         mb_init(mb_full, 1u);
@@ -727,9 +810,12 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const int g0 = d.sysoff[s];
         const int N_s = d.sysoff[s + 1] - g0;
         const int N8 = (N_s + 7) & ~7;
-        const int A_s = ((((N_s + CL - 1) / CL) + 3) >> 2) << 2;
+        const int A_s = ((((N_s + CL - 1) / CL) + 7) >> 3) << 3;   /* whole blocks of eight slots per CTA */
         const int a_begin = rank * A_s;
         const int A_own = max(0, min(A_s, N_s - a_begin));
+        const int sb0 = min(a_begin, N8), sbw = min(a_begin + A_s, N8) - sb0;   /* the CTA's own slots [sb0, sb0 + sbw) */
+        const int n_peer_slots = N8 - sbw;            /* slots of the other CTAs */
+        const unsigned peer_bytes = (unsigned)(N_s - A_own) * SB;
         const SysGeom &geo = d.geom[s];
         int fstat0 = 0;
         if (FIRE) {                                    /* finished systems stay bit-unchanged (R22) */
@@ -787,13 +873,16 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         T hdt = (T)c.hdt, dt = (T)c.dt;
         int n_done = 0;                               /* steps taken by this system in this call */
         bool have_ev = false;                         /* the last pair pass also produced E (and W) */
+        MARK(100);
         cluster.sync();                               /* constants visible; previous system fully retired everywhere */
+        MARK(101);
 
 #ifdef TS_RES_TIMING
         long long prof_acc[12] = { 0 }, prof_t = clock64();
 #endif
         for (int n = 0; n <= n_steps; ++n) {
             bool rebuild = n == 0;
+            const bool last = n == n_steps;
             if (FIRE && n > 0) {
                 if (fsm->nsteps >= fp.max_steps) {     /* reported as failed, never counted (R24) */
                     __syncthreads();
@@ -804,6 +893,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             }
             if (n > 0) {
                 bool moved = false;
+                if (tid == 0 && peer_bytes) mb_expect_tx(mb_full, peer_bytes);   /* this step's home slots of the other CTAs */
                 if (own) {
                     /* first half of the step (O3 / O4), as in the general engine */
                     if (FIRE || c.integrator == TS_NVE) {
@@ -825,27 +915,36 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     T a = x0 - r0, b = x1 - r1, cc = x2 - r2;
                     moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
                 }
-                TICK(0);
-                if (!FIRE) cl_wait();                 /* every CTA of the cluster has finished reading the old positions (FIRE: fire_reduce's barriers) */
-                TICK(1);
-                if (tid == 0) mb_expect_tx(mb_full, (unsigned)N_s * (unsigned)(4 * sizeof(T)));   /* this step's home slots */
+                if (!FIRE && CL > 1) cl_wait();       /* every CTA of the cluster has finished reading the old positions (FIRE: fire_reduce's barriers) */
                 if (own) {
+                    /* the new home slot: into the other CTAs' slot arrays with st.async, which completes transaction bytes
+                     * on the RECEIVING CTA's mbarrier (the skin flag travels in the type word); into the own slot array
+                     * directly, together with the images of the atom */
                     const T px = x0 - ws0, py = x1 - ws1, pz = x2 - ws2;
-                    const int tyw = ty | (moved ? MOVED_BIT : 0);         /* the skin flag travels with the slot */
+                    const int tyw = ty | (moved ? MOVED_BIT : 0);
                     for (int r = 0; r < CL; ++r)
-                        st_async_pos(map_cluster(pos_sa + (unsigned)hs * 16u, (unsigned)r), map_cluster(mb_full, (unsigned)r), zt, px, py, pz, tyw);
+                        if (r != rank)
+                            st_async_pos(map_cluster(pos_sa + (unsigned)hs * 16u, (unsigned)r), map_cluster(mb_full, (unsigned)r), zt, px, py, pz, tyw);
+                    st_pos(posb, (unsigned)hs * 16u, zt, px, py, pz, ty);
+                    ghost_write<T>(posb, zt, gtab[hs], gh, px, py, pz, ty);
                 }
-                TICK(2);
-                mb_wait(mb_full, full_parity);        /* all home slots of the step have arrived in THIS CTA */
-                full_parity ^= 1u;
+                TICK(0);
+                if (peer_bytes) {                     /* all home slots of the others have arrived in THIS CTA */
+                    mb_wait(mb_full, full_parity);
+                    full_parity ^= 1u;
+                }
                 TICK(3);
-                /* images of the new home positions (local) and the owners' skin flags */
-                rebuild = __syncthreads_or(ghost_pass<T>(posb, zt, gtab, gh, N_s) ? 1 : 0) != 0;
+                /* images of the others' new home positions and their skin flags; own home and image slots complete */
+                moved |= peer_pass<T>(posb, zt, gtab, gh, sb0, sbw, n_peer_slots, N_s);
+                rebuild = __syncthreads_or(moved ? 1 : 0) != 0;
+                TICK(4);
             }
             if (rebuild) {
                 /* every CTA of the cluster takes this branch in the same step (the flags travel with the home slots);
                  * nobody may still be reading its home / ghost slots when the re-wrapped slots and fr arrive */
+                MARK(1);
                 cluster.sync();
+                MARK(2);
                 if (tid == 0) { misc->rebuilds += 1u; misc->nnz = 0u; }
                 if (own) {
                     /* wrap into the cell: f = x . h^-1, w = floor(f) (R5: the stored x stays unwrapped) */
@@ -869,26 +968,30 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     const T far = (T)1e15;
                     st_pos(posb, (unsigned)(N8 + tid) * 16u, zt, far, far, far, 0);
                 }
+                MARK(3);
                 cluster.sync();                       /* fractions and home slots complete in every CTA */
-                TICK(4);
-                ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
                 TICK(5);
+                MARK(4);
+                ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
                 TICK(6);
-                build_phase(rc, fr, gtab, rows, cnt, G, G[6], a_begin, A_own, N_s, N8, misc);
+                MARK(5);
+                build_phase(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc);
                 __syncthreads();
                 TICK(7);
+                MARK(6);
                 ghost_pass<T>(posb, zt, gtab, gh, N_s);          /* images again: the rebuild re-wrapped the home slots */
                 __syncthreads();
+                TICK(8);
+                MARK(7);
             }
-            TICK(10);
-            const bool last = n == n_steps;
-            if (last) pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
-            else pair_phase<T, KIND, NT1, false>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
+            if (last) pair_phase<T, KIND, NT1, true>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
+            else pair_phase<T, KIND, NT1, false>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
             have_ev = last;
-            TICK(8);
-            if (!FIRE) cl_arrive_relaxed();           /* this CTA no longer reads the positions of step n */
-            __syncthreads();
             TICK(9);
+            if (!FIRE && CL > 1) cl_arrive_relaxed(); /* this CTA no longer reads the positions of step n */
+            __syncthreads();
+            TICK(10);
+            MARK(9);
             if (own) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
                 if (n > 0) { v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im); }
@@ -941,9 +1044,9 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 }
             }
         }
-        if (!FIRE) cl_wait();                         /* pairs the last arrive */
+        if (!FIRE && CL > 1) cl_wait();               /* pairs the last arrive */
         if (FIRE && !have_ev) {                       /* stopped before the last pass: E of the final positions */
-            pair_phase<T, KIND, NT1, true>(rc, posb, rows, cnt, tab, fs, a_begin, A_own, N8, NT, red);
+            pair_phase<T, KIND, NT1, true>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
             __syncthreads();
         }
 #ifdef TS_RES_TIMING
@@ -1016,11 +1119,11 @@ static unsigned up16(unsigned x) { return (x + 15u) & ~15u; }
 static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types, int thread_div = 1)
 {
     size_t w = dtype == TS_F32 ? 4 : 8;
-    int A = ((((nmax + CL - 1) / CL) + 3) / 4) * 4;
+    int A = ((((nmax + CL - 1) / CL) + 7) / 8) * 8;              /* whole blocks of eight slots per CTA */
     int max_threads = (dtype == TS_F32 ? RES_MAX_THREADS : RES_MAX_THREADS_F64) / thread_div;
     if (getenv("TS_RES_MAXT")) max_threads = atoi(getenv("TS_RES_MAXT"));
     if (A > max_threads) return false;
-    int pitch = 32 * ((need_row + 31) / 32);                     /* whole trips of 32 entries */
+    int pitch = 16 * ((need_row + 15) / 16);                     /* whole trips of 16 entries */
     int ntasks = A / 4, maxw = max_threads / 32;
     int passes = (ntasks + maxw - 1) / maxw;
     int nwarps = (ntasks + passes - 1) / passes;
@@ -1036,7 +1139,7 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.o_gtab = o; o += up16((unsigned)nmax * 4u);
     c.o_rows = o; o += up16((unsigned)A * (unsigned)pitch * 2u);
     c.o_fs = o; o += up16((unsigned)(3 * A * w));
-    c.o_cnt = o; o += up16((unsigned)A * 4u);
+    c.o_meta = o; o += up16((unsigned)A * 4u);                    /* one word per atom slot of a task */
     c.o_pot = o; o += up16((unsigned)(n_types * n_types * (dtype == TS_F32 ? sizeof(PotEntry<float>) : sizeof(PotEntry<double>))));
     c.o_red = o; o += (unsigned)(RES_MAX_THREADS / 32) * 64u;
     c.o_cred = o; o += 8u * 64u;
