@@ -85,8 +85,9 @@ struct ResCfg {
     int NS;            /* position slots per CTA: atoms + dummies + ghosts     */
     int nwarps;
     int n_clusters;
-    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_meta, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
+    unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_own, o_meta, o_noise, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
     unsigned smem;
+    int noise_helpers; /* the kick buffers of the noise helpers exist (they are left out when they do not fit) */
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
 };
 
@@ -101,6 +102,7 @@ struct ResMisc {
 /* optional phase timers (build with -DTS_RES_TIMING; debugging only): cycles of warp 0 of every CTA */
 #ifdef TS_RES_TIMING
 __device__ unsigned long long g_res_prof[16];
+__device__ unsigned long long g_res_wprof[64];   /* [0..31] pair-phase cycles per warp, [32..63] trips per warp */
 #define TICK(k) do { if (threadIdx.x == 0) { long long t__ = clock64(); prof_acc[k] += t__ - prof_t; prof_t = t__; } } while (0)
 #else
 #define TICK(k) do { } while (0)
@@ -152,6 +154,11 @@ __device__ __forceinline__ void st_async_pos(unsigned dst, unsigned bar, unsigne
 
 /* ------------------------------------------------------------------ position slots */
 template <typename T> struct P3 { T x, y, z; int ty; };
+template <typename T> struct __align__(16) Q4 { T a, b, c, d; };
+__device__ __forceinline__ float bits_to(int v, float) { return __int_as_float(v); }
+__device__ __forceinline__ double bits_to(int v, double) { return __longlong_as_double((long long)v); }
+__device__ __forceinline__ int bits_from(float v) { return __float_as_int(v); }
+__device__ __forceinline__ int bits_from(double v) { return (int)__double_as_longlong(v); }
 
 __device__ __forceinline__ P3<float> ld_pos(const unsigned char *base, unsigned off, unsigned, float)
 {
@@ -333,6 +340,12 @@ __device__ __forceinline__ float4 lds128(unsigned a)
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
     return v;
 }
+__device__ __forceinline__ uint2 lds64(unsigned a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ unsigned lds32(unsigned a)
 {
     unsigned v;
@@ -366,8 +379,10 @@ __device__ __forceinline__ void lj_pair2(const float4 &pa, const float4 &pb, flo
     float r2a, r2b;
     upk2(R2, r2a, r2b);
     float ia, ib;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
+    /* volatile: keeps the arithmetic of a pair behind the (volatile) gathers issued before it in program order, so
+     * that the gathers of the next two entries are in flight while this pair is computed */
+    asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));
+    asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
     const float ma = r2a < rc2 ? 1.0f : 0.0f, mb = r2b < rc2 ? 1.0f : 0.0f;   /* strict (R9) */
     const f32x2 I = mul2(pk2(ia, ib), pk2(ma, mb));
     const f32x2 I2 = mul2(I, I);
@@ -380,12 +395,19 @@ __device__ __forceinline__ void lj_pair2(const float4 &pa, const float4 &pb, flo
 }
 
 /* ------------------------------------------------------------------ list layout
- * The list of the four atoms of a task (one warp: quarter-warp q = atom, lane l = column = 16-byte bank group) is a
- * sequence of TRIPS of 128 bytes: lane (q, l) owns the 32-bit word at q * 32 + l * 4, which holds two entries (list
- * rows 2 t and 2 t + 1 of column l).  An entry is the number of a position slot (14 bits): the even row sits in bits
- * 0..13, the odd row in bits 18..31, bits 14..17 are zero, so that the shared-memory address of the odd slot is one
- * instruction (base + (word >> 14): LEA.HI) and the even one two (mask; base + 16 x: IMAD).  tmeta[4 task + q] =
- * home slot of the atom | trips << 14 (the trip count is the same for the four atoms of a task). */
+ * A TASK is eight consecutive own atoms, served by one warp: four lanes per atom (lane = 4 a + l4, a = atom of the
+ * task, l4 = lane of the atom).  The list of an atom has eight COLUMNS, one per 16-byte bank group of the slot array
+ * (column c holds neighbours whose slot number is c modulo 8), and R rows; lane l4 reads the columns l4 and l4 + 4.
+ * The list of a task is a sequence of TRIPS of 256 bytes: lane (a, l4) owns the 64-bit word at a * 32 + l4 * 8, which
+ * holds four entries, gathered in the order k = 0..3:
+ *     k = 0: row 2 t,     column l4 + 4 p        k = 1: row 2 t,     column l4 + 4 (1 - p)
+ *     k = 2: row 2 t + 1, column l4 + 4 p        k = 3: row 2 t + 1, column l4 + 4 (1 - p)        p = a & 1
+ * so that the eight lanes of a quarter-warp (two atoms of opposite parity) gather from eight different bank groups in
+ * every step: one shared-memory wavefront per quarter-warp unless a group overflowed its column (build_phase).
+ * An entry is the number of a position slot (14 bits): k = 0, 2 sit in bits 0..13 of the two 32-bit halves, k = 1, 3
+ * in bits 18..31, bits 14..17 are zero, so that the shared-memory address of an odd entry is one instruction (base +
+ * (word >> 14): LEA.HI) and of an even one two (mask; base + 16 x: IMAD).  tmeta[8 task + a] = home slot of the atom |
+ * trips << 14 (the trip count is the same for the eight atoms of a task). */
 #define ENT_MASK 0x3fffu
 __device__ __forceinline__ unsigned ent_even(unsigned w, unsigned base)
 {
@@ -395,24 +417,22 @@ __device__ __forceinline__ unsigned ent_even(unsigned w, unsigned base)
 }
 __device__ __forceinline__ unsigned ent_odd(unsigned w, unsigned base) { return base + (w >> 14); }
 
-/* sum over the eight lanes of an atom of three values in four shuffles: lanes 0-1 end with fx, 2-3 fy, 4-5 fz */
+/* sum over the four lanes of an atom of three values in three shuffles: lane 0 ends with fx, 1 fy, 2 fz (3: zero) */
 template <typename T>
-__device__ __forceinline__ T reduce3_8(T fx, T fy, T fz, int l)
+__device__ __forceinline__ T reduce3_4(T fx, T fy, T fz, int l4)
 {
-    const bool h4 = (l & 4) != 0, h2 = (l & 2) != 0;
-    const T r0 = __shfl_xor_sync(0xffffffffu, h4 ? fx : fz, 4);
-    const T r1 = __shfl_xor_sync(0xffffffffu, fy, 4);
-    T a = (h4 ? fz : fx) + r0;                    /* lanes 0-3: fx of lanes {l, l ^ 4}; lanes 4-7: fz */
-    T b = h4 ? (T)0 : fy + r1;                    /* lanes 0-3: fy */
-    const T r2 = __shfl_xor_sync(0xffffffffu, h2 ? a : b, 2);
-    T v = (h2 ? b : a) + r2;                      /* lanes 0,1: fx; 2,3: fy; 4,5: fz; 6,7: 0 */
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    return v;
+    const bool h = (l4 & 2) != 0, o = (l4 & 1) != 0;
+    const T r0 = __shfl_xor_sync(0xffffffffu, h ? fx : fz, 2);
+    const T r1 = __shfl_xor_sync(0xffffffffu, fy, 2);
+    const T a = (h ? fz : fx) + r0;               /* lanes 0-1: fx of lanes {l, l ^ 2}; lanes 2-3: fz */
+    const T b = h ? (T)0 : fy + r1;               /* lanes 0-1: fy */
+    const T r2 = __shfl_xor_sync(0xffffffffu, o ? a : b, 1);
+    return (o ? b : a) + r2;
 }
 
 /* Forces of the CTA's own atoms from the shared-memory list; EV: energy and virial partials accumulate in fp64 (R31)
- * and end as warp partials in red.  FAST = fp32 Lennard-Jones, one type, forces only: the two entries of a word
- * share packed f32x2 operations, and the positions of trip t + 1 are gathered while trip t is computed. */
+ * and end as warp partials in red.  FAST = fp32 Lennard-Jones, one type, forces only: two entries share packed f32x2
+ * operations, and the positions of the next two entries are gathered while the current two are computed. */
 template <typename T, int KIND, bool NT1, bool EV>
 __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, unsigned rows_sa, const unsigned *tmeta,
                                            const PotEntry<T> *tab, T *fs, int A_own, int NT, double *red)
@@ -422,19 +442,19 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
 #pragma unroll
         for (int k = 0; k < 7; ++k) acc[k] = 0.0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int l = lane & 7, q = lane >> 3;
+    const int l4 = lane & 3, a8 = lane >> 2;
     const unsigned zt = (unsigned)rc.NS * 16u;
-    const int ntasks = (A_own + 3) >> 2;
+    const int ntasks = (A_own + 7) >> 3;
     constexpr bool FAST = (sizeof(T) == 4) && KIND == TS_LJ && NT1 && !EV;
-    const unsigned task_stride = (unsigned)rc.pitch * 8u;
-    const unsigned lane_off = (unsigned)q * 32u + (unsigned)l * 4u;
+    const unsigned task_stride = (unsigned)rc.pitch * 16u;
+    const unsigned lane_off = (unsigned)lane * 8u;
     const PotEntry<T> pe1 = tab[0];
     const float rc2f = (float)pe1.rc2, m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
-        const unsigned meta = tmeta[task * 4 + q];
+        const int al = task * 8 + a8;
+        const unsigned meta = tmeta[al];
         const int nt = (int)(meta >> 14);
         const unsigned xa = pos_sa + ((meta & ENT_MASK) << 4);
-        const int al = task * 4 + q;
         const bool has = al < A_own;
         const unsigned ra = rows_sa + (unsigned)task * task_stride + lane_off;
         T fx = 0, fy = 0, fz = 0;
@@ -445,16 +465,18 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
             const f32x2 C12 = pk2(m12, m12), C6 = pk2(p6, p6);
             f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
             if (nt > 0) {
-                unsigned w = lds32(ra);
-                float4 p0 = lds128(ent_even(w, pos_sa)), p1 = lds128(ent_odd(w, pos_sa));
-                w = lds32(ra + 128u);                                    /* one word past the list is still inside shared memory */
+                uint2 w = lds64(ra);
+                float4 p0 = lds128(ent_even(w.x, pos_sa)), p1 = lds128(ent_odd(w.x, pos_sa));
                 for (int t = 1; t < nt; ++t) {
-                    const float4 q0 = lds128(ent_even(w, pos_sa)), q1 = lds128(ent_odd(w, pos_sa));
-                    w = lds32(ra + (unsigned)(t + 1) * 128u);
+                    const float4 q0 = lds128(ent_even(w.y, pos_sa)), q1 = lds128(ent_odd(w.y, pos_sa));
+                    w = lds64(ra + (unsigned)t * 256u);
                     lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
-                    p0 = q0; p1 = q1;
+                    p0 = lds128(ent_even(w.x, pos_sa)); p1 = lds128(ent_odd(w.x, pos_sa));
+                    lj_pair2(q0, q1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
                 }
+                const float4 q0 = lds128(ent_even(w.y, pos_sa)), q1 = lds128(ent_odd(w.y, pos_sa));
                 lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
+                lj_pair2(q0, q1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
             }
             float a, b;
             upk2(FX, a, b); fx = (T)(a + b);
@@ -464,17 +486,20 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
             const P3<T> xi = ld_pos_sa(xa, zt, (T)0);
             const PotEntry<T> pei = NT1 ? pe1 : tab[xi.ty * NT];
             const int tirow = xi.ty * NT;
-            unsigned w = lds32(ra);
             for (int t = 0; t < nt; ++t) {
-                const P3<T> x0 = ld_pos_sa(ent_even(w, pos_sa), zt, (T)0);
-                const P3<T> x1 = ld_pos_sa(ent_odd(w, pos_sa), zt, (T)0);
-                w = lds32(ra + (unsigned)(t + 1) * 128u);
+                const uint2 w = lds64(ra + (unsigned)t * 256u);
+                const P3<T> x0 = ld_pos_sa(ent_even(w.x, pos_sa), zt, (T)0);
+                const P3<T> x1 = ld_pos_sa(ent_odd(w.x, pos_sa), zt, (T)0);
+                const P3<T> x2 = ld_pos_sa(ent_even(w.y, pos_sa), zt, (T)0);
+                const P3<T> x3 = ld_pos_sa(ent_odd(w.y, pos_sa), zt, (T)0);
                 pair_accum<T, KIND, NT1, EV>(xi, x0, pei, tab, tirow, fx, fy, fz, ev);
                 pair_accum<T, KIND, NT1, EV>(xi, x1, pei, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x2, pei, tab, tirow, fx, fy, fz, ev);
+                pair_accum<T, KIND, NT1, EV>(xi, x3, pei, tab, tirow, fx, fy, fz, ev);
             }
         }
-        const T v = reduce3_8<T>(fx, fy, fz, l);
-        if (has && l < 6 && !(l & 1)) fs[(l >> 1) * rc.A + al] = v;
+        const T v = reduce3_4<T>(fx, fy, fz, l4);
+        if (has && l4 < 3) fs[l4 * rc.A + al] = v;
         if (EV && has) {                /* fp64 from here on (R31): E = 1/2 sum V, W = -1/2 sum g r (x) r */
             acc[0] += 0.5 * (double)ev[0];
 #pragma unroll
@@ -556,7 +581,7 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
-    const int ntasks = (A_own + 3) >> 2;
+    const int ntasks = (A_own + 7) >> 3;          /* tasks of the pair phase: eight atoms, built four at a time */
     const f32x2 G0 = pk2(G[0], G[0]), G1 = pk2(G[1], G[1]), G2 = pk2(G[2], G[2]);
     const f32x2 G3 = pk2(G[3], G[3]), G4 = pk2(G[4], G[4]), G5 = pk2(G[5], G[5]);
     const bool ovf = misc->overflow != 0;         /* ghost slots exhausted: leave every row empty (flagged) */
@@ -564,7 +589,11 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
     const int W = (T + 31) >> 5;                  /* mask words per lane */
     unsigned nnz = 0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
-        const int al = task * 4 + q;
+      int Rh0 = 0, Rh1 = 0, ai0 = 0;
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        const int a8 = half * 4 + q;                            /* atom of the task */
+        const int al = task * 8 + a8;
         const bool has = al < A_own;
         const int ai = hslot(a_begin + (has ? al : 0), N8);     /* slot of the atom: the build works in slot space */
         const uint4 ui = fr[ai];
@@ -618,17 +647,19 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
         for (int c = 0; c < 8; ++c) cq[c] = __shfl_sync(0xffffffffu, mine, c, 8);
         int R = ((NT + 15) >> 4) << 1;                                /* rows: whole trips of 16 entries */
         R = max(R, __shfl_xor_sync(0xffffffffu, R, 8));
-        R = max(R, __shfl_xor_sync(0xffffffffu, R, 16));              /* the four atoms of a task share the loop counts */
+        R = max(R, __shfl_xor_sync(0xffffffffu, R, 16));              /* the four atoms of a half task place into the same rows */
         const bool fits = 8 * R <= rc.pitch && !ovf;
         if (!fits) {
             if (lane == 0) misc->overflow = 1;
             R = 0;
         }
-        /* u16 halves of the trip words of this atom: row r of column c lives at base + (r / 2) * 64 + c * 2 + (r & 1);
+        /* u16 halves of the trip words of this atom (see "list layout"): row r of column c lives at
+         * base + (r / 2) * 128 + (c & 3) * 4 + (r & 1) * 2 + ((c >> 2) ^ p), p = parity of the atom in its task;
          * the odd half holds the entry << 2 (bits 18..31 of the word) */
-        unsigned short *rowB = rows + (size_t)task * rc.pitch * 4 + q * 16;
-#define CELL_B(r, c) rowB[((r) >> 1) * 64 + (c) * 2 + ((r) & 1)]
-#define ENT(slot, r) (unsigned short)((unsigned)(slot) << (((r) & 1) << 1))
+        unsigned short *rowB = rows + (size_t)task * rc.pitch * 8 + a8 * 16;
+        const int par = a8 & 1;
+#define CELL_B(r, c) rowB[((r) >> 1) * 128 + ((c) & 3) * 4 + ((r) & 1) * 2 + (((c) >> 2) ^ par)]
+#define ENT(slot, c) (unsigned short)((unsigned)(slot) << (((((c) >> 2) ^ par)) << 1))
         if (fits) {
             /* Placement.  The pair loop reads R rows of eight entries; entry (row, column) is read by lane
              * `column`, and one shared-memory wavefront serves a row when its eight bank groups differ.  Lane l
@@ -681,17 +712,31 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
                         prow = cc + (u - Fc);
                         ++u;
                     }
-                    CELL_B(prow, pcol) = ENT(slot, prow);
+                    CELL_B(prow, pcol) = ENT(slot, pcol);
                     ++m;
                 }
             }
             /* padding of my column below my own hits and the overflow entries it received */
-            for (int r = min(mine, R) + recv; r < R; ++r) CELL_B(r, l) = ENT(N8 + l, r);
+            for (int r = min(mine, R) + recv; r < R; ++r) CELL_B(r, l) = ENT(N8 + l, l);
+        }
+        if (half == 0) { Rh0 = R; ai0 = has ? ai : N8; } else Rh1 = R;
+        if (has) nnz += (unsigned)mine;
+        if (half == 1) {
+            /* the eight atoms of the task share the trip count: the shorter half is padded with dummies */
+            const int Rm = max(Rh0, Rh1);
+            unsigned short *row0 = rows + (size_t)task * rc.pitch * 8 + q * 16;
+            const int par0 = q & 1;
+            for (int r = Rh0; r < Rm; ++r)
+                row0[(r >> 1) * 128 + (l & 3) * 4 + (r & 1) * 2 + ((l >> 2) ^ par0)] = (unsigned short)((unsigned)(N8 + l) << (((l >> 2) ^ par0) << 1));
+            for (int r = Rh1; r < Rm; ++r) CELL_B(r, l) = ENT(N8 + l, l);
+            if (l == 0) {
+                tmeta[task * 8 + q] = (unsigned)ai0 | ((unsigned)(Rm >> 1) << 14);
+                tmeta[task * 8 + 4 + q] = (unsigned)(has ? ai : N8) | ((unsigned)(Rm >> 1) << 14);
+            }
         }
 #undef CELL_B
 #undef ENT
-        if (l == 0) tmeta[task * 4 + q] = (unsigned)(has ? ai : N8) | ((unsigned)(R >> 1) << 14);
-        if (has) nnz += (unsigned)mine;
+      }
     }
     nnz = __reduce_add_sync(0xffffffffu, nnz);
     if (lane == 0 && nnz) atomicAdd(&misc->nnz, nnz);
@@ -785,6 +830,14 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     unsigned short *rows = (unsigned short *)(smem + rc.o_rows);
     T *fs = (T *)(smem + rc.o_fs);
     unsigned *tmeta = (unsigned *)(smem + rc.o_meta);
+    T *noise = (T *)(smem + rc.o_noise);  /* [2][3][A] */
+    /* state of the own atoms, one 4-vector each, between the owner phases.  fp32: in shared memory -- at 72 registers
+     * per thread (864 threads) the registers belong to the pair loop, whose gathers must stay one trip ahead of its
+     * arithmetic.  fp64 (512 threads, 128 registers): in registers (Xr, Vr, Rr), the slots are twice as large */
+    constexpr bool OWN_SMEM = sizeof(T) == 4;
+    Q4<T> *ox = (Q4<T> *)(smem + rc.o_own);   /* [A] x (unwrapped), 1 / (m mass_conv)                                 */
+    Q4<T> *ov = ox + rc.A;                    /* [A] v                                                                */
+    Q4<T> *oref = ov + rc.A;                  /* [A] x at the last build (skin test), packed wrap shift (wa, wb, wc)   */
     PotEntry<T> *tab = (PotEntry<T> *)(smem + rc.o_pot);
     double *red = (double *)(smem + rc.o_red);
     double *cred = (double *)(smem + rc.o_cred);
@@ -857,19 +910,30 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const int ai = a_begin + tid;                 /* system-local atom index  */
         const int hs = hslot(ai, N8);                 /* its home slot            */
         const long long gi = (long long)g0 + ai;      /* global atom index        */
-        T x0 = 0, x1 = 0, x2 = 0, v0 = 0, v1 = 0, v2 = 0, f0 = 0, f1 = 0, f2 = 0, r0 = 0, r1 = 0, r2 = 0;
-        T ws0 = 0, ws1 = 0, ws2 = 0, im = 0, mass = 0;
         int ty = 0;
+        Q4<T> Xr, Vr, Rr;
+        Xr.a = Xr.b = Xr.c = Xr.d = 0; Vr = Xr; Rr = Xr;
         if (own) {
             const T *x = (const T *)d.pos + 3 * gi, *v = (const T *)d.vel + 3 * gi;
-            x0 = x[0]; x1 = x[1]; x2 = x[2]; v0 = v[0]; v1 = v[1]; v2 = v[2];
-            mass = ((const T *)d.mass)[gi];
-            im = (T)1 / (mass * (T)d.mass_conv);
+            Q4<T> X, V;
+            X.a = x[0]; X.b = x[1]; X.c = x[2]; V.a = v[0]; V.b = v[1]; V.c = v[2]; V.d = 0;
+            X.d = (T)1 / (((const T *)d.mass)[gi] * (T)d.mass_conv);
             ty = d.type[gi];
-            if (FIRE && fstat0 == TS_FIRE_FRESH) { v0 = 0; v1 = 0; v2 = 0; }
+            if (FIRE && fstat0 == TS_FIRE_FRESH) { V.a = 0; V.b = 0; V.c = 0; }
+            if (OWN_SMEM) { ox[tid] = X; ov[tid] = V; } else { Xr = X; Vr = V; }
         }
         const unsigned uid = d.uid_own[s];
         const unsigned long long step0 = d.sys_step[s];
+        /* Langevin noise (O4, O5): when the block has a spare thread for every own atom, thread blockDim - A_own + k draws
+         * the kick c2 sqrt(kT / m) xi of atom k for step n + 1 while the owners integrate step n: the Philox rounds and the
+         * Box-Muller transform are more than half of the owners' dependent instruction chain */
+        const bool noise_helpers = !FIRE && rc.noise_helpers && c.integrator == TS_BAOAB && (int)blockDim.x >= 2 * A_own;
+        const int hk = tid - ((int)blockDim.x - A_own);          /* helper of own atom hk */
+        T hsig = 0;
+        if (noise_helpers && hk >= 0) {
+            const T hm = (T)1 / (((const T *)d.mass)[g0 + a_begin + hk] * (T)d.mass_conv);
+            hsig = (T)c.c2 * (sizeof(T) == 4 ? (T)sqrtf((float)((T)c.kT * hm)) : (T)sqrt((double)((T)c.kT * hm)));
+        }
         T hdt = (T)c.hdt, dt = (T)c.dt;
         int n_done = 0;                               /* steps taken by this system in this call */
         bool have_ev = false;                         /* the last pair pass also produced E (and W) */
@@ -891,15 +955,37 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 }
                 dt = (T)fsm->dt; hdt = (T)0.5 * dt;
             }
+            if (noise_helpers && hk >= 0 && n < n_steps) {             /* the kicks of step n + 1 */
+                const unsigned long long step = step0 + (unsigned long long)n;
+                unsigned w[4];
+                philox4x32_10((unsigned)(a_begin + hk), uid, (unsigned)(step & 0xffffffffull), (unsigned)(step >> 32), c.key0, c.key1, w);
+                T xi[3];
+                normals3(w, xi);
+                T *nz = noise + ((n + 1) & 1) * 3 * rc.A + hk;
+                nz[0] = hsig * xi[0]; nz[rc.A] = hsig * xi[1]; nz[2 * rc.A] = hsig * xi[2];
+            }
             if (n > 0) {
                 bool moved = false;
                 if (tid == 0 && peer_bytes) mb_expect_tx(mb_full, peer_bytes);   /* this step's home slots of the other CTAs */
+                T x0 = 0, x1 = 0, x2 = 0;
+                int wpack = 0;
                 if (own) {
+                    const T f0 = fs[tid], f1 = fs[rc.A + tid], f2 = fs[2 * rc.A + tid];
+                    const Q4<T> X = OWN_SMEM ? ox[tid] : Xr, V = OWN_SMEM ? ov[tid] : Vr, R = OWN_SMEM ? oref[tid] : Rr;
+                    const T im = X.d;
+                    T v0 = V.a, v1 = V.b, v2 = V.c;
+                    x0 = X.a; x1 = X.b; x2 = X.c;
                     /* first half of the step (O3 / O4), as in the general engine */
                     if (FIRE || c.integrator == TS_NVE) {
                         v0 = v0 + hdt * (f0 * im); x0 = x0 + dt * v0;
                         v1 = v1 + hdt * (f1 * im); x1 = x1 + dt * v1;
                         v2 = v2 + hdt * (f2 * im); x2 = x2 + dt * v2;
+                    } else if (noise_helpers) {
+                        const T *nz = noise + (n & 1) * 3 * rc.A + tid;
+                        const T c1 = (T)c.c1, k0 = nz[0], k1 = nz[rc.A], k2 = nz[2 * rc.A];
+                        v0 = v0 + hdt * (f0 * im); x0 = x0 + hdt * v0; v0 = c1 * v0 + k0; x0 = x0 + hdt * v0;
+                        v1 = v1 + hdt * (f1 * im); x1 = x1 + hdt * v1; v1 = c1 * v1 + k1; x1 = x1 + hdt * v1;
+                        v2 = v2 + hdt * (f2 * im); x2 = x2 + hdt * v2; v2 = c1 * v2 + k2; x2 = x2 + hdt * v2;
                     } else {
                         unsigned long long step = step0 + (unsigned long long)(n - 1);
                         unsigned w[4];
@@ -912,15 +998,25 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                         v1 = v1 + hdt * (f1 * im); x1 = x1 + hdt * v1; v1 = c1 * v1 + c2 * sig * xi[1]; x1 = x1 + hdt * v1;
                         v2 = v2 + hdt * (f2 * im); x2 = x2 + hdt * v2; v2 = c1 * v2 + c2 * sig * xi[2]; x2 = x2 + hdt * v2;
                     }
-                    T a = x0 - r0, b = x1 - r1, cc = x2 - r2;
+                    Q4<T> Xn, Vn;
+                    Xn.a = x0; Xn.b = x1; Xn.c = x2; Xn.d = im; Vn.a = v0; Vn.b = v1; Vn.c = v2; Vn.d = 0;
+                    if (OWN_SMEM) { ox[tid] = Xn; ov[tid] = Vn; } else { Xr = Xn; Vr = Vn; }
+                    T a = x0 - R.a, b = x1 - R.b, cc = x2 - R.c;
                     moved = (double)(a * a + b * b + cc * cc) > d.half_skin2;
+                    wpack = bits_from(R.d);
                 }
+                TICK(1);
                 if (!FIRE && CL > 1) cl_wait();       /* every CTA of the cluster has finished reading the old positions (FIRE: fire_reduce's barriers) */
+                TICK(2);
                 if (own) {
                     /* the new home slot: into the other CTAs' slot arrays with st.async, which completes transaction bytes
                      * on the RECEIVING CTA's mbarrier (the skin flag travels in the type word); into the own slot array
                      * directly, together with the images of the atom */
-                    const T px = x0 - ws0, py = x1 - ws1, pz = x2 - ws2;
+                    /* the wrap shift of the last build, from its integer coefficients with the expression of the build */
+                    const T wa = (T)(signed char)(wpack & 0xff), wb = (T)(signed char)((wpack >> 8) & 0xff), wc = (T)(signed char)((wpack >> 16) & 0xff);
+                    const T px = x0 - (wa * gh[0] + wb * gh[3] + wc * gh[6]);
+                    const T py = x1 - (wa * gh[1] + wb * gh[4] + wc * gh[7]);
+                    const T pz = x2 - (wa * gh[2] + wb * gh[5] + wc * gh[8]);
                     const int tyw = ty | (moved ? MOVED_BIT : 0);
                     for (int r = 0; r < CL; ++r)
                         if (r != rank)
@@ -948,6 +1044,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 if (tid == 0) { misc->rebuilds += 1u; misc->nnz = 0u; }
                 if (own) {
                     /* wrap into the cell: f = x . h^-1, w = floor(f) (R5: the stored x stays unwrapped) */
+                    const Q4<T> X = OWN_SMEM ? ox[tid] : Xr;
+                    const T x0 = X.a, x1 = X.b, x2 = X.c;
                     T fa = x0 * gh[9] + x1 * gh[12] + x2 * gh[15];
                     T fb = x0 * gh[10] + x1 * gh[13] + x2 * gh[16];
                     T fc = x0 * gh[11] + x1 * gh[14] + x2 * gh[17];
@@ -956,10 +1054,15 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     if (fa >= (T)1) { wa += (T)1; fa = (T)0; }
                     if (fb >= (T)1) { wb += (T)1; fb = (T)0; }
                     if (fc >= (T)1) { wc += (T)1; fc = (T)0; }
-                    ws0 = wa * gh[0] + wb * gh[3] + wc * gh[6];
-                    ws1 = wa * gh[1] + wb * gh[4] + wc * gh[7];
-                    ws2 = wa * gh[2] + wb * gh[5] + wc * gh[8];
-                    r0 = x0; r1 = x1; r2 = x2;
+                    const T ws0 = wa * gh[0] + wb * gh[3] + wc * gh[6];
+                    const T ws1 = wa * gh[1] + wb * gh[4] + wc * gh[7];
+                    const T ws2 = wa * gh[2] + wb * gh[5] + wc * gh[8];
+                    /* |w| < 128, or the system is flagged: an atom that far outside its cell has left any sensible trajectory */
+                    if (!(fabs((double)wa) < 127.5 && fabs((double)wb) < 127.5 && fabs((double)wc) < 127.5)) atomicOr(&d.status->flags, TS_FLAG_SHIFT_RANGE);
+                    Q4<T> R;
+                    R.a = x0; R.b = x1; R.c = x2;
+                    R.d = bits_to(((int)wa & 0xff) | (((int)wb & 0xff) << 8) | (((int)wc & 0xff) << 16), (T)0);
+                    if (OWN_SMEM) oref[tid] = R; else Rr = R;
                     const uint4 u = make_uint4(frac_to_u32(fa), frac_to_u32(fb), frac_to_u32(fc), 0u);
                     for (int r = 0; r < CL; ++r) cluster.map_shared_rank(fr, r)[hs] = u;
                     publish_home<T>(cluster, CL, posb, zt, hs, x0 - ws0, x1 - ws1, x2 - ws2, ty);
@@ -984,17 +1087,35 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 TICK(8);
                 MARK(7);
             }
+#ifdef TS_RES_TIMING
+            const long long wt0 = clock64();
+#endif
             if (last) pair_phase<T, KIND, NT1, true>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
             else pair_phase<T, KIND, NT1, false>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
+#ifdef TS_RES_TIMING
+            if ((tid & 31) == 0) {
+                atomicAdd(&g_res_wprof[tid >> 5], (unsigned long long)(clock64() - wt0));
+                unsigned tr = 0;
+                for (int task = tid >> 5; task < (A_own + 7) / 8; task += rc.nwarps) tr += tmeta[task * 8] >> 14;
+                atomicAdd(&g_res_wprof[32 + (tid >> 5)], (unsigned long long)tr);
+            }
+#endif
             have_ev = last;
             TICK(9);
             if (!FIRE && CL > 1) cl_arrive_relaxed(); /* this CTA no longer reads the positions of step n */
             __syncthreads();
             TICK(10);
             MARK(9);
-            if (own) {
+            T f0 = 0, f1 = 0, f2 = 0, v0 = 0, v1 = 0, v2 = 0;
+            if (own && (FIRE || n > 0)) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
-                if (n > 0) { v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im); }
+                const Q4<T> V = OWN_SMEM ? ov[tid] : Vr;
+                v0 = V.a; v1 = V.b; v2 = V.c;
+                if (n > 0) {
+                    const T im = OWN_SMEM ? ox[tid].d : Xr.d;
+                    v0 = v0 + hdt * (f0 * im); v1 = v1 + hdt * (f1 * im); v2 = v2 + hdt * (f2 * im);
+                    if (!FIRE) { Q4<T> Vn; Vn.a = v0; Vn.b = v1; Vn.c = v2; Vn.d = 0; if (OWN_SMEM) ov[tid] = Vn; else Vr = Vn; }
+                }
             }
             if (n > 0) n_done = n;
             if (FIRE) {
@@ -1021,6 +1142,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                             }
                         } else if (own) { v0 = 0; v1 = 0; v2 = 0; }
                     }
+                    if (own) { Q4<T> Vn; Vn.a = v0; Vn.b = v1; Vn.c = v2; Vn.d = 0; if (OWN_SMEM) ov[tid] = Vn; else Vr = Vn; }
                     __syncthreads();                  /* everybody has read the state of this step */
                     if (tid == 0) {
                         fsm->nsteps += 1;
@@ -1056,8 +1178,11 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         double ke = 0.0;
         if (own) {
             T *x = (T *)d.pos + 3 * gi, *v = (T *)d.vel + 3 * gi, *f = (T *)d.force + 3 * gi;
+            const T f0 = fs[tid], f1 = fs[rc.A + tid], f2 = fs[2 * rc.A + tid];
+            const Q4<T> X = OWN_SMEM ? ox[tid] : Xr, V = OWN_SMEM ? ov[tid] : Vr;
+            const T x0 = X.a, x1 = X.b, x2 = X.c, v0 = V.a, v1 = V.b, v2 = V.c;
             x[0] = x0; x[1] = x1; x[2] = x2; v[0] = v0; v[1] = v1; v[2] = v2; f[0] = f0; f[1] = f1; f[2] = f2;
-            ke = 0.5 * (double)mass * d.mass_conv * ((double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2);
+            ke = 0.5 * (double)((const T *)d.mass)[gi] * d.mass_conv * ((double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2);
             if (!(fabs((double)f0) + fabs((double)f1) + fabs((double)f2) < 1e300)) atomicOr(&d.status->flags, TS_FLAG_NONFINITE);
         }
         const double tot = reduce8(cluster, CL, rank, ke, red, cred, rc.nwarps);
@@ -1116,7 +1241,7 @@ static ResKernel pick_kernel(const ts_state *st, bool fire = false)
 static unsigned up16(unsigned x) { return (x + 15u) & ~15u; }
 
 /* Shared-memory carve for cluster size CL; returns false when it does not fit. */
-static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types, int thread_div = 1)
+static bool res_layout_n(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types, int thread_div, int with_noise)
 {
     size_t w = dtype == TS_F32 ? 4 : 8;
     int A = ((((nmax + CL - 1) / CL) + 7) / 8) * 8;              /* whole blocks of eight slots per CTA */
@@ -1139,7 +1264,10 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.o_gtab = o; o += up16((unsigned)nmax * 4u);
     c.o_rows = o; o += up16((unsigned)A * (unsigned)pitch * 2u);
     c.o_fs = o; o += up16((unsigned)(3 * A * w));
+    c.o_own = o; o += dtype == TS_F32 ? up16((unsigned)(12 * A * w)) : 0u;   /* fp32: x | 1/m, v, x_ref | wrap shift of the own atoms */
     c.o_meta = o; o += up16((unsigned)A * 4u);                    /* one word per atom slot of a task */
+    c.noise_helpers = with_noise;
+    c.o_noise = o; o += with_noise ? up16((unsigned)(6 * A * w)) : 0u;   /* Langevin kicks of the own atoms, two steps */
     c.o_pot = o; o += up16((unsigned)(n_types * n_types * (dtype == TS_F32 ? sizeof(PotEntry<float>) : sizeof(PotEntry<double>))));
     c.o_red = o; o += (unsigned)(RES_MAX_THREADS / 32) * 64u;
     c.o_cred = o; o += 8u * 64u;
@@ -1148,6 +1276,13 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     c.o_mbar = o; o += 16u;                                       /* FULL mbarrier of the position exchange */
     c.smem = o;
     return o <= RES_SMEM_LIMIT;
+}
+
+/* with the kick buffers of the noise helpers when they fit, else without */
+static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots, int dtype, int n_types, int thread_div = 1)
+{
+    if (res_layout_n(c, CL, nmax, need_row, need_slots, dtype, n_types, thread_div, 1)) return true;
+    return res_layout_n(c, CL, nmax, need_row, need_slots, dtype, n_types, thread_div, 0);
 }
 
 /* Decides once per batch geometry whether the resident engine applies and how it is launched. */
@@ -1317,6 +1452,12 @@ extern "C" int ts_debug_resident_profile(unsigned long long *out16)
     unsigned long long z[16] = { 0 };
     if (cudaMemcpyFromSymbol(out16, g_res_prof, sizeof z) != cudaSuccess) return 1;
     cudaMemcpyToSymbol(g_res_prof, z, sizeof z);
+    if (getenv("TS_RES_WPROF")) {
+        unsigned long long w[64], zz[64] = { 0 };
+        cudaMemcpyFromSymbol(w, g_res_wprof, sizeof w);
+        cudaMemcpyToSymbol(g_res_wprof, zz, sizeof zz);
+        for (int k = 0; k < 32; ++k) fprintf(stderr, "warp %2d pair cycles %llu trips %llu\n", k, w[k], w[32 + k]);
+    }
     return 0;
 #else
     (void)out16;
