@@ -9,33 +9,40 @@
  *                    ALL atoms of the system (a hashed permutation of the atom order, hslot), eight
  *                    far-away dummies (list padding, one per 16-byte bank group) and the GHOST
  *                    slots: every periodic image of an atom that can lie within r_list of the cell
- *                    owns a slot holding x + S.h, in the bank group of its atom.  Owners publish
- *                    only their home slot into every CTA of the cluster through DSMEM; every CTA
- *                    regenerates the ghosts locally each step (ghost_pass).
+ *                    owns a slot holding x + S.h, in the bank group of its atom.  An owner writes the
+ *                    home slot and the images of its atom locally and sends the home slot to the
+ *                    other CTAs of the cluster through DSMEM; every CTA regenerates the images of
+ *                    the other CTAs' atoms locally each step (peer_pass).
  *     fr[N_s]        fractional coordinates as 32-bit fixed point (rebuilds only; aliased onto the
- *                    ghost slots, which are dead between the cluster barrier of a step and the ghost
- *                    refresh after a rebuild)
+ *                    ghost slots, which are dead between the cluster barrier of a rebuild and the
+ *                    ghost refresh that ends it)
  *     gtab[N_s]      first ghost slot, active axes and image signs of every atom
- *     rows[A][pitch] the Verlet list of the CTA's own atoms: 16-bit entries = slot number of the
- *                    neighbour.  Thanks to the ghosts EVERY pair is a plain difference of two slots:
- *                    no image arithmetic in the pair loop.  One COLUMN per bank group (build_phase).
+ *     rows           the Verlet list of the CTA's own atoms: 14-bit entries = slot number of the
+ *                    neighbour, in trips of 16 entries per atom (see "list layout").  Thanks to the
+ *                    ghosts EVERY pair is a plain difference of two slots: no image arithmetic in the
+ *                    pair loop.  One COLUMN per bank group (build_phase).
  *     fs[3][A]       forces of the own atoms (pair phase -> integrator phase)
- * and in registers of the owner thread of an atom: x (unwrapped), v, F, x_ref, wrap shift.  HBM is
- * touched when a system is loaded, when it is stored, and never in between.
+ *     own state      fp32: x (unwrapped) | 1/m, v, x_ref | wrap shift of the own atoms as three
+ *                    4-vectors per atom (the 72 registers of a thread belong to the pair loop);
+ *                    fp64: the same in registers of the owner thread
+ * HBM is touched when a system is loaded, when it is stored, and never in between.
  *
- * One MD step = [owner: B A (O A) + skin test] -> wait(peers done reading; split-phase cluster
- * barrier, no fence) -> [publish home slots with st.async: they complete transaction bytes on the
- * receiving CTA's mbarrier, the skin flag rides in the slot's type word] -> wait on the own mbarrier
- * -> [ghost refresh] -> [rebuild if any atom moved > skin/2, then ghosts again] -> [pair phase] ->
- * arrive(done reading) -> block barrier -> [owner: B].  FIRE mode (template flag): per-system dt,
- * the four reductions and the state machine after every step, finished systems skipped untouched.
- * Same physics as the general engine.
+ * One MD step = [owner: B A (O A) + skin test; spare threads draw the Langevin kicks of the next
+ * step] -> wait(peers done reading; split-phase cluster barrier, no fence) -> [home slots to the
+ * other CTAs with st.async: they complete transaction bytes on the receiving CTA's mbarrier, the
+ * skin flag rides in the slot's type word; own home slot and images locally] -> wait on the own
+ * mbarrier -> [images of the others' atoms] -> [rebuild if any atom moved > skin/2, then all images
+ * again] -> [pair phase] -> arrive(done reading) -> block barrier -> [owner: B].  FIRE mode
+ * (template flag): per-system dt, the four reductions and the state machine after every step,
+ * finished systems skipped untouched.  Same physics as the general engine (SURVEY O2..O6, R5, R9,
+ * R12, R16, R18, R21, R22).
  *
- * Pair phase: 8 lanes per atom (one quarter-warp = one LDS.128 phase), rows read in trips of 32
- * entries (one 64-bit load per lane).  Lane l of the builder tests the slots = l mod 8, so a lane's
- * hits all live in 16-byte bank group l and fill column l of the atom's list: a row of eight is
- * served by one shared-memory wavefront unless a group overflowed its column.  The fp32
- * Lennard-Jones force-only loop uses Blackwell's packed FFMA2/FMUL2 (f32x2) on pairs of pairs.
+ * Pair phase: tasks of eight atoms per warp, four lanes per atom; the two atoms of a quarter-warp
+ * gather from eight different 16-byte bank groups in every step ("list layout").  The builder's
+ * lane l tests the slots = l mod 8, so its hits all live in bank group l and fill column l of the
+ * atom's list: a gather is served by one shared-memory wavefront per quarter-warp unless a group
+ * overflowed its column.  The fp32 Lennard-Jones force-only loop uses Blackwell's packed
+ * FFMA2/FMUL2 (f32x2) on pairs of entries and gathers two entries ahead of the arithmetic.
  *
  * Rebuild: brute force over the system in fractional fixed point (integer subtraction wraps = the
  * minimum image), valid because the engine is only used when every cell height is >= 2 r_list
@@ -55,22 +62,6 @@
 #include "ts_rng.cuh"
 
 namespace cg = cooperative_groups;
-#ifdef DBG_MARK
-__device__ volatile int *g_dbg;
-__device__ __forceinline__ unsigned dbg_chk(unsigned a, unsigned fallback, int code, unsigned x0, unsigned x1)
-{
-    if (a >= 136000u || (a & 15u)) {
-        if (g_dbg) { int k = 64 + 8 * (int)(blockIdx.x & 3); if (g_dbg[k] == 0) { g_dbg[k] = code; g_dbg[k + 1] = (int)a; g_dbg[k + 2] = (int)x0; g_dbg[k + 3] = (int)x1; g_dbg[k + 4] = threadIdx.x; } }
-        return fallback;
-    }
-    return a;
-}
-#define CHK(a, fb, code, x0, x1) dbg_chk(a, fb, code, x0, x1)
-#define WMARK(code) do { if (g_dbg && (threadIdx.x & 31) == 0) { g_dbg[128 + 32 * (blockIdx.x & 3) + (threadIdx.x >> 5)] = (code); __threadfence_system(); } } while (0)
-#else
-#define WMARK(code) do { } while (0)
-#define CHK(a, fb, code, x0, x1) (a)
-#endif
 
 #define RES_MAX_THREADS 896         /* fp32; the fp64 kernels need twice the registers: 512 */
 #define RES_MAX_THREADS_F64 512
@@ -805,12 +796,6 @@ __device__ __forceinline__ void fire_reduce(cg::cluster_group &cluster, int CL, 
     if (CL > 1) cluster.sync(); else __syncthreads();          /* cred may be rewritten by the next reduction */
 }
 
-#ifdef DBG_MARK
-extern "C" int ts_debug_set_marker(int *p) { return (int)cudaMemcpyToSymbol(g_dbg, &p, sizeof p); }
-#define MARK(k) do { __syncthreads(); if (g_dbg && threadIdx.x == 0) { g_dbg[blockIdx.x] = (k); __threadfence_system(); } } while (0)
-#else
-#define MARK(k) do { } while (0)
-#endif
 /* ------------------------------------------------------------------ the kernel */
 template <typename T, int KIND, bool NT1, bool FIRE>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THREADS_F64, 1) k_resident_md(DevState d, MdConst c, ResCfg rc, int n_steps, unsigned want, ts_fire_params fp)
@@ -830,7 +815,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     unsigned short *rows = (unsigned short *)(smem + rc.o_rows);
     T *fs = (T *)(smem + rc.o_fs);
     unsigned *tmeta = (unsigned *)(smem + rc.o_meta);
-    T *noise = (T *)(smem + rc.o_noise);  /* [2][3][A] */
+    T *noise = (T *)(smem + rc.o_noise);  /* [3][A] Langevin kicks of the own atoms for the next step */
     /* state of the own atoms, one 4-vector each, between the owner phases.  fp32: in shared memory -- at 72 registers
      * per thread (864 threads) the registers belong to the pair loop, whose gathers must stay one trip ahead of its
      * arithmetic.  fp64 (512 threads, 128 registers): in registers (Xr, Vr, Rr), the slots are twice as large */
@@ -937,9 +922,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         T hdt = (T)c.hdt, dt = (T)c.dt;
         int n_done = 0;                               /* steps taken by this system in this call */
         bool have_ev = false;                         /* the last pair pass also produced E (and W) */
-        MARK(100);
         cluster.sync();                               /* constants visible; previous system fully retired everywhere */
-        MARK(101);
 
 #ifdef TS_RES_TIMING
         long long prof_acc[12] = { 0 }, prof_t = clock64();
@@ -955,14 +938,15 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 }
                 dt = (T)fsm->dt; hdt = (T)0.5 * dt;
             }
-            if (noise_helpers && hk >= 0 && n < n_steps) {             /* the kicks of step n + 1 */
+            T kick0 = 0, kick1 = 0, kick2 = 0;
+            const bool draws = noise_helpers && hk >= 0 && n < n_steps;
+            if (draws) {                                               /* the kicks of step n + 1, stored once the owners have read those of step n */
                 const unsigned long long step = step0 + (unsigned long long)n;
                 unsigned w[4];
                 philox4x32_10((unsigned)(a_begin + hk), uid, (unsigned)(step & 0xffffffffull), (unsigned)(step >> 32), c.key0, c.key1, w);
                 T xi[3];
                 normals3(w, xi);
-                T *nz = noise + ((n + 1) & 1) * 3 * rc.A + hk;
-                nz[0] = hsig * xi[0]; nz[rc.A] = hsig * xi[1]; nz[2 * rc.A] = hsig * xi[2];
+                kick0 = hsig * xi[0]; kick1 = hsig * xi[1]; kick2 = hsig * xi[2];
             }
             if (n > 0) {
                 bool moved = false;
@@ -981,7 +965,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                         v1 = v1 + hdt * (f1 * im); x1 = x1 + dt * v1;
                         v2 = v2 + hdt * (f2 * im); x2 = x2 + dt * v2;
                     } else if (noise_helpers) {
-                        const T *nz = noise + (n & 1) * 3 * rc.A + tid;
+                        const T *nz = noise + tid;
                         const T c1 = (T)c.c1, k0 = nz[0], k1 = nz[rc.A], k2 = nz[2 * rc.A];
                         v0 = v0 + hdt * (f0 * im); x0 = x0 + hdt * v0; v0 = c1 * v0 + k0; x0 = x0 + hdt * v0;
                         v1 = v1 + hdt * (f1 * im); x1 = x1 + hdt * v1; v1 = c1 * v1 + k1; x1 = x1 + hdt * v1;
@@ -1035,12 +1019,11 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 rebuild = __syncthreads_or(moved ? 1 : 0) != 0;
                 TICK(4);
             }
+            if (draws) { noise[hk] = kick0; noise[rc.A + hk] = kick1; noise[2 * rc.A + hk] = kick2; }
             if (rebuild) {
                 /* every CTA of the cluster takes this branch in the same step (the flags travel with the home slots);
                  * nobody may still be reading its home / ghost slots when the re-wrapped slots and fr arrive */
-                MARK(1);
                 cluster.sync();
-                MARK(2);
                 if (tid == 0) { misc->rebuilds += 1u; misc->nnz = 0u; }
                 if (own) {
                     /* wrap into the cell: f = x . h^-1, w = floor(f) (R5: the stored x stays unwrapped) */
@@ -1071,21 +1054,16 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     const T far = (T)1e15;
                     st_pos(posb, (unsigned)(N8 + tid) * 16u, zt, far, far, far, 0);
                 }
-                MARK(3);
                 cluster.sync();                       /* fractions and home slots complete in every CTA */
                 TICK(5);
-                MARK(4);
                 ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
                 TICK(6);
-                MARK(5);
                 build_phase(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc);
                 __syncthreads();
                 TICK(7);
-                MARK(6);
                 ghost_pass<T>(posb, zt, gtab, gh, N_s);          /* images again: the rebuild re-wrapped the home slots */
                 __syncthreads();
                 TICK(8);
-                MARK(7);
             }
 #ifdef TS_RES_TIMING
             const long long wt0 = clock64();
@@ -1105,7 +1083,6 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             if (!FIRE && CL > 1) cl_arrive_relaxed(); /* this CTA no longer reads the positions of step n */
             __syncthreads();
             TICK(10);
-            MARK(9);
             T f0 = 0, f1 = 0, f2 = 0, v0 = 0, v1 = 0, v2 = 0;
             if (own && (FIRE || n > 0)) {
                 f0 = fs[tid]; f1 = fs[rc.A + tid]; f2 = fs[2 * rc.A + tid];
@@ -1267,7 +1244,7 @@ static bool res_layout_n(ResCfg &c, int CL, int nmax, int need_row, int need_slo
     c.o_own = o; o += dtype == TS_F32 ? up16((unsigned)(12 * A * w)) : 0u;   /* fp32: x | 1/m, v, x_ref | wrap shift of the own atoms */
     c.o_meta = o; o += up16((unsigned)A * 4u);                    /* one word per atom slot of a task */
     c.noise_helpers = with_noise;
-    c.o_noise = o; o += with_noise ? up16((unsigned)(6 * A * w)) : 0u;   /* Langevin kicks of the own atoms, two steps */
+    c.o_noise = o; o += with_noise ? up16((unsigned)(3 * A * w)) : 0u;   /* Langevin kicks of the own atoms for the next step */
     c.o_pot = o; o += up16((unsigned)(n_types * n_types * (dtype == TS_F32 ? sizeof(PotEntry<float>) : sizeof(PotEntry<double>))));
     c.o_red = o; o += (unsigned)(RES_MAX_THREADS / 32) * 64u;
     c.o_cred = o; o += 8u * 64u;
