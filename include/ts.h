@@ -26,8 +26,11 @@
  *  - Calls are asynchronous on `stream` unless stated.  A ts_state is not thread-safe.
  *  - Errors: argument errors return immediately (nothing enqueued).  Conditions found on the device
  *    (neighbour capacity overflow, image shift out of range, non-finite force, bad cell) set sticky
- *    bits in a device status word; ts_poll reports them and every later stepping call returns
- *    TS_ERR_STICKY until ts_clear_error.  On overflow nothing is written past capacity.
+ *    bits in a device status word; ts_poll reports them, and once ts_poll has observed them every later
+ *    stepping call returns TS_ERR_STICKY until ts_clear_error.  On overflow nothing is written past capacity.
+ *  - Synchronising calls: ts_workspace_bytes, ts_state_create, ts_poll, ts_converged_mask, ts_swap_systems,
+ *    ts_repack_systems, ts_get_neighbors, ts_set/get_system_steps, ts_clear_error; the first stepping call of the
+ *    resident engine after create or after a swap / repack with new cells reads the cell geometry back once.
  *  - No CPU fallback exists: every entry point needs a CUDA device.
  */
 #ifndef TS_H
@@ -120,13 +123,13 @@ typedef struct {
 
 typedef struct {
     uint32_t flags;          /* TS_FLAG_* sticky bits */
-    int32_t n_rebuilds;      /* neighbour builds since create */
+    int32_t n_rebuilds;      /* general engine: build events since create in which at least one system was rebuilt */
     int64_t nnz;             /* directed pairs in the current list (resident engine: summed over the systems' lists) */
     int64_t nnz_capacity;
     int64_t steps_done;      /* MD/FIRE steps enqueued since create */
     int32_t n_converged;     /* systems with FIRE status converged */
     int32_t n_failed;        /* systems that hit max_steps */
-    int32_t max_neighbors;   /* longest row of the current list (general engine) */
+    int32_t max_neighbors;   /* longest row built since the last full build (general engine; a running maximum over per-system rebuilds) */
     int32_t list_valid;
     int64_t resident_rebuilds; /* resident engine: per-system list builds since create, summed over systems */
     int32_t engine;          /* engine that ran the last stepping call: 0 general, 1 resident */
@@ -151,7 +154,9 @@ ts_status ts_state_create(const ts_state_desc *desc, const ts_potential *pot,
 ts_status ts_state_destroy(ts_state *st);
 
 /* Cell-list neighbour build from the current desc.pos: binning + counting sort by
- * (system, cell), count -> scan -> capacity check -> fill of the CSR list at radius max rc + skin. */
+ * (system, cell), then ONE search pass that buffers each row, reserves its place in the system's CSR
+ * segment with one atomic and copies it out (rows of any length; capacity check per system: on
+ * overflow nothing is written past the segment, TS_FLAG_NBR_OVERFLOW is set and the list is invalid). */
 ts_status ts_build_neighbors(ts_state *st, void *stream);
 
 /* Forces (always), energy / virial when asked from the current desc.pos; rebuilds
@@ -177,18 +182,58 @@ ts_status ts_poll(ts_state *st, ts_report *out, void *stream);
 ts_status ts_converged_mask(ts_state *st, uint8_t *mask, int32_t *status, int32_t *fire_steps,
                             void *stream);
 
-/* In-flight swap: replace the systems in `slots` (HOST, n entries) by the
+/* In-flight swap, equal sizes (ts_repack_systems: any sizes).  Synchronises `stream`; the
+ * stepping call that follows a swap with new cells re-plans the resident engine (one small device read).
+ * Replaces the systems in `slots` (HOST, n entries) by the
  * n systems of `fresh` (device arrays pos, vel, mass, type, cell, sys_uid; system k of fresh must
  * have exactly as many atoms as slot slots[k]).  Their FIRE state becomes fresh, their step
  * counter 0, and the neighbour list is marked stale.                                              */
 ts_status ts_swap_systems(ts_state *st, const int32_t *slots, int32_t n, const ts_state_desc *fresh,
                           void *stream);
 
+/* Ragged in-flight replacement (Fig. 3): the batch becomes the systems
+ * keep[0..n_keep) of the current batch (HOST slot numbers, each at most once, in the order given) followed by the
+ * systems of `fresh` (device arrays pos, vel (NULL: zero), mass, type, cell, sys_uid (NULL: slot number);
+ * fresh_n_atoms HOST [fresh->n_systems]; NULL fresh: compaction only), of any sizes.  Kept systems keep positions,
+ * velocities, FIRE state, step counters and uids; fresh ones start FRESH at step 0.  n_atoms, n_systems and the
+ * neighbour list are re-laid; energy / virial / kinetic of a slot are stale until the next force evaluation.  The new
+ * batch must fit what the state was created with (ts_get_capacity: atoms, systems, pair slots), else
+ * TS_ERR_WORKSPACE_TOO_SMALL and nothing has changed.  Synchronises `stream`.                                      */
+ts_status ts_repack_systems(ts_state *st, const int32_t *keep, int32_t n_keep, const ts_state_desc *fresh,
+                            const int32_t *fresh_n_atoms, void *stream);
+
+/* Capacity of a state (sizes at create) and the pair slots one system needs (the paper's n_atoms x density scaler,
+ * PAPER.md:88, with the coefficient the library uses): what an admission rule has to add up before a repack.       */
+ts_status ts_get_capacity(const ts_state *st, int64_t *n_atoms, int32_t *n_systems, int64_t *n_pairs);
+ts_status ts_estimate_system_pairs(int64_t n_atoms, double volume, double r_list, double slack, int64_t *out_pairs);
+
 /* Synchronising export of the current list to HOST arrays (test / graph export): off [N+1], and
  * for each directed pair its GLOBAL neighbour index j and image shift S (relative to the stored
  * positions, R6).  cap = capacity of j / shift in pairs; TS_ERR_WORKSPACE_TOO_SMALL if nnz > cap. */
 ts_status ts_get_neighbors(ts_state *st, int64_t *off, int32_t *j, int8_t *shift, int64_t cap,
                            void *stream);
+
+/* ---- graph export and external-model stepping (SURVEY 8(f) NEXT-2; PAPER.md:56 ModelInterface, :112) ------------
+ * The current Verlet list (radius max rc + skin, general engine; built or skin-checked first) as a dense edge list in
+ * DEVICE arrays: edge_i / edge_j [cap] global atom indices, edge_shift [cap,3] in the state dtype = the integer image
+ * shift S of the pair: r_ij = x_j - x_i + S . h with the STORED positions (R6).  *n_edges (device) = edges of the
+ * list; when it exceeds cap only the first cap edges are written.  Edges of a system are contiguous, systems in batch
+ * order.  Asynchronous on `stream`.                                                                                 */
+ts_status ts_export_edges(ts_state *st, int64_t *edge_i, int64_t *edge_j, void *edge_shift, int64_t cap,
+                          int64_t *n_edges, void *stream);
+
+/* One MD / FIRE step split around a force evaluation the CALLER enqueues on `stream` (an external energies / forces /
+ * stress provider writing desc.force, and desc.energy / desc.virial if it wants them reported):
+ *   MD:   TS_PHASE_INIT (list for the current positions) -> caller: F(x) -> then per step
+ *         TS_PHASE_PRE (B A (O A), skin check, rebuild if due: ts_export_edges is current) -> caller: F(x) ->
+ *         TS_PHASE_POST (B, kinetic energy, step counters += 1).
+ *   FIRE: TS_PHASE_INIT (fresh systems: v = 0, dt_start, alpha_start; list) -> caller: F(x) -> TS_PHASE_CHECK0 (the
+ *         0-step convergence test) -> per step TS_PHASE_PRE -> caller: F(x) -> TS_PHASE_POST (second half kick,
+ *         reductions, FIRE state machine; frozen systems stay bit-unchanged).
+ * Same integrator kernels as ts_md_step / ts_fire_step of the general engine.  Asynchronous.                         */
+enum { TS_PHASE_INIT = 0, TS_PHASE_PRE = 1, TS_PHASE_POST = 2, TS_PHASE_CHECK0 = 3 };
+ts_status ts_md_step_external(ts_state *st, const ts_md_params *p, int32_t phase, void *stream);
+ts_status ts_fire_step_external(ts_state *st, const ts_fire_params *p, int32_t phase, void *stream);
 
 /* Per-system step counters used by the Philox counter (R18): HOST [S] in / out.  Synchronising.   */
 ts_status ts_set_system_steps(ts_state *st, const uint64_t *steps, void *stream);

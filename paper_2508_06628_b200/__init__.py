@@ -30,7 +30,12 @@ EXPORTS = ["ts_workspace_bytes", "ts_estimate_system_bytes", "ts_state_create", 
            "ts_converged_mask", "ts_swap_systems", "ts_get_neighbors", "ts_set_system_steps",
            "ts_get_system_steps", "ts_set_engine", "ts_invalidate", "ts_launch_count", "ts_clear_error",
            "ts_status_string", "ts_last_error", "ts_sched_fill", "ts_sched_max_scaler",
-           "ts_sched_binpack", "ts_sched_partition"]
+           "ts_sched_binpack", "ts_sched_partition", "ts_repack_systems", "ts_get_capacity",
+           "ts_estimate_system_pairs", "ts_export_edges", "ts_md_step_external", "ts_fire_step_external"]
+
+TS_PHASE_INIT, TS_PHASE_PRE, TS_PHASE_POST, TS_PHASE_CHECK0 = 0, 1, 2, 3
+(TS_OK, TS_ERR_INVALID_ARG, TS_ERR_CUDA, TS_ERR_WORKSPACE_TOO_SMALL, TS_ERR_NBR_OVERFLOW, TS_ERR_STALE_NBR,
+ TS_ERR_NONFINITE, TS_ERR_UNSUPPORTED, TS_ERR_STICKY) = range(9)
 
 
 class ts_units(C.Structure):
@@ -177,6 +182,40 @@ def ts_swap_systems(h, slots, fresh_desc):
     slots = np.ascontiguousarray(np.asarray(slots, dtype=np.int32))
     _check(lib().ts_swap_systems(h, slots.ctypes.data_as(C.c_void_p), C.c_int32(slots.size), C.byref(fresh_desc),
                                  _stream()), "ts_swap_systems", h)
+
+
+def ts_repack_systems(h, keep, fresh_desc, fresh_n_atoms):
+    keep = np.ascontiguousarray(np.asarray(keep, dtype=np.int32))
+    fn = np.ascontiguousarray(np.asarray(fresh_n_atoms, dtype=np.int32))
+    _check(lib().ts_repack_systems(h, keep.ctypes.data_as(C.c_void_p), C.c_int32(keep.size),
+                                   C.byref(fresh_desc) if fresh_desc is not None else None,
+                                   fn.ctypes.data_as(C.c_void_p), _stream()), "ts_repack_systems", h)
+
+
+def ts_get_capacity(h):
+    n, s, p = C.c_int64(), C.c_int32(), C.c_int64()
+    _check(lib().ts_get_capacity(h, C.byref(n), C.byref(s), C.byref(p)), "ts_get_capacity", h)
+    return n.value, s.value, p.value
+
+
+def ts_estimate_system_pairs(n_atoms, volume, r_list, slack=1.25):
+    out = C.c_int64()
+    _check(lib().ts_estimate_system_pairs(C.c_int64(int(n_atoms)), C.c_double(volume), C.c_double(r_list),
+                                          C.c_double(slack), C.byref(out)), "ts_estimate_system_pairs")
+    return out.value
+
+
+def ts_export_edges(h, edge_i_ptr, edge_j_ptr, edge_shift_ptr, cap, n_edges_ptr):
+    _check(lib().ts_export_edges(h, C.c_void_p(edge_i_ptr), C.c_void_p(edge_j_ptr), C.c_void_p(edge_shift_ptr),
+                                 C.c_int64(cap), C.c_void_p(n_edges_ptr), _stream()), "ts_export_edges", h)
+
+
+def ts_md_step_external(h, params, phase):
+    _check(lib().ts_md_step_external(h, C.byref(params), C.c_int32(phase), _stream()), "ts_md_step_external", h)
+
+
+def ts_fire_step_external(h, params, phase):
+    _check(lib().ts_fire_step_external(h, C.byref(params), C.c_int32(phase), _stream()), "ts_fire_step_external", h)
 
 
 def ts_get_neighbors(h, n_atoms):

@@ -65,7 +65,7 @@ TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types
 
 /* Pair slots reserved for a system of n atoms in volume vol: the paper's n_atoms_x_density
  * scaler (section 3) with a known coefficient: n * rho * 4/3 pi r_list^3 * slack. */
-static long long system_pair_capacity(long long n, double vol, double r_list, double slack)
+long long ts_system_pair_capacity(long long n, double vol, double r_list, double slack)
 {
     if (slack < 1.0) slack = 1.25;
     double nbar = (double)n / vol * (4.0 / 3.0) * M_PI * r_list * r_list * r_list;
@@ -95,7 +95,7 @@ extern "C" ts_status ts_estimate_system_bytes(int64_t n_atoms, double volume, do
     size_t boundary = (size_t)n_atoms * (3 * 3 * w + w + 4 + 4) + 9 * w + 8 * 11 + 4;
     size_t per_sys = sizeof(SysGeom) + 9 * w + 8 * 2 + 8 * 2 + 4 * 5 /* incl. sys_rebuild */ + 32 + 8 + 4 + 8 + 4 * 2 /* cell slots */;
     size_t ws = (size_t)n_atoms * per_atom_workspace_bytes(dtype) + per_sys +
-                4 * (size_t)system_pair_capacity(n_atoms, volume, r_list, slack);
+                4 * (size_t)ts_system_pair_capacity(n_atoms, volume, r_list, slack);
     *out_bytes = boundary + ws;
     return TS_OK;
 }
@@ -151,7 +151,7 @@ static ts_status scan_batch(const ts_state_desc *d, const ts_potential *pot, con
                      h[2] * (h[3] * h[7] - h[4] * h[6]);
         if (!(fabs(det) > 0.0)) return TS_ERR_INVALID_ARG;
         long long n = sysoff[(size_t)s + 1] - sysoff[(size_t)s];
-        nbr_base[(size_t)s + 1] = nbr_base[(size_t)s] + system_pair_capacity(n, fabs(det), r_list, nbr->slack);
+        nbr_base[(size_t)s + 1] = nbr_base[(size_t)s] + ts_system_pair_capacity(n, fabs(det), r_list, nbr->slack);
     }
     return TS_OK;
 }
@@ -218,6 +218,7 @@ extern "C" ts_status ts_state_create(const ts_state_desc *desc, const ts_potenti
     st->desc = *desc;
     st->nbr = *nbr;
     st->engine = 1;
+    st->N_cap = N; st->S_cap = S;
     st->h_sysoff = (int *)malloc(sizeof(int) * (size_t)(S + 1));
     memcpy(st->h_sysoff, sysoff.data(), sizeof(int) * (size_t)(S + 1));
     char *ws = (char *)workspace;
@@ -244,28 +245,33 @@ extern "C" ts_status ts_state_create(const ts_state_desc *desc, const ts_potenti
     d.nbr_cnt = (int *)(ws + L.nbr_cnt); d.nbr_off = (long long *)(ws + L.nbr_off);
     d.nbr = (unsigned int *)(ws + L.nbr); d.nbr_cap = base.back();
 
+#define CREATE_OK(call)                                                                   \
+    do {                                                                                  \
+        if ((call) != cudaSuccess) { free(st->h_sysoff); free(st); return TS_ERR_CUDA; }  \
+    } while (0)
     /* everything up to the per-pair region starts zeroed (FIRE status FRESH = 0, steps 0, flags 0) */
-    TS_CUDA_OK(st, cudaMemset(ws, 0, L.nbr));
-    TS_CUDA_OK(st, cudaMemcpy(d.sysoff, sysoff.data(), sizeof(int) * (size_t)(S + 1), cudaMemcpyHostToDevice));
-    TS_CUDA_OK(st, cudaMemcpy(d.nbr_base, base.data(), sizeof(long long) * (size_t)(S + 1), cudaMemcpyHostToDevice));
+    CREATE_OK(cudaMemset(ws, 0, L.nbr));
+    CREATE_OK(cudaMemcpy(d.sysoff, sysoff.data(), sizeof(int) * (size_t)(S + 1), cudaMemcpyHostToDevice));
+    CREATE_OK(cudaMemcpy(d.nbr_base, base.data(), sizeof(long long) * (size_t)(S + 1), cudaMemcpyHostToDevice));
     std::vector<char> pbuf;
     if (desc->dtype == TS_F32) fill_pot<float>(pot, pbuf); else fill_pot<double>(pot, pbuf);
-    TS_CUDA_OK(st, cudaMemcpy(d.pot, pbuf.data(), pbuf.size(), cudaMemcpyHostToDevice));
+    CREATE_OK(cudaMemcpy(d.pot, pbuf.data(), pbuf.size(), cudaMemcpyHostToDevice));
     if (desc->sys_uid) {
-        TS_CUDA_OK(st, cudaMemcpy(d.uid_own, desc->sys_uid, sizeof(unsigned) * (size_t)S, cudaMemcpyDeviceToDevice));
+        CREATE_OK(cudaMemcpy(d.uid_own, desc->sys_uid, sizeof(unsigned) * (size_t)S, cudaMemcpyDeviceToDevice));
     } else {
         std::vector<unsigned> iota((size_t)S);
         for (int s = 0; s < S; ++s) iota[(size_t)s] = (unsigned)s;
-        TS_CUDA_OK(st, cudaMemcpy(d.uid_own, iota.data(), sizeof(unsigned) * (size_t)S, cudaMemcpyHostToDevice));
+        CREATE_OK(cudaMemcpy(d.uid_own, iota.data(), sizeof(unsigned) * (size_t)S, cudaMemcpyHostToDevice));
     }
     launch_geometry(st, 0, S, nullptr, 0);
-    TS_CUDA_OK(st, cudaDeviceSynchronize());
+    CREATE_OK(cudaDeviceSynchronize());
     DevStatus hs;
-    TS_CUDA_OK(st, cudaMemcpy(&hs, d.status, sizeof hs, cudaMemcpyDeviceToHost));
+    CREATE_OK(cudaMemcpy(&hs, d.status, sizeof hs, cudaMemcpyDeviceToHost));
     if (hs.flags & TS_FLAG_BAD_CELL) {
         free(st->h_sysoff); free(st);
         return TS_ERR_INVALID_ARG;
     }
+#undef CREATE_OK
     *out = st;
     return TS_OK;
 }

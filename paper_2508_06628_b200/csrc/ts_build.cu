@@ -211,7 +211,8 @@ __device__ __forceinline__ int floordiv(int a, int n) { int q = a / n; return (a
  * and share their loads.  The lanes of a quarter stride over the atoms of each stencil bin; hits are compacted with a
  * quarter-wide ballot into a shared-memory buffer (NBR_BUF entries per atom).  When the walk is done the quarter
  * reserves a contiguous row inside the CSR segment of its system with one atomicAdd on the system's cursor (nbr_len)
- * and copies the row out: no counting pass, no scan.  Rows of a system are therefore stored in arrival order (nbr_off
+ * and copies the row out: no counting pass, no scan (a row longer than the buffer is walked a second time and written
+ * straight into the reserved place).  Rows of a system are therefore stored in arrival order (nbr_off
  * says where); the content and order of every row are deterministic.  Nothing is written past the capacity of the
  * segment: a row that does not fit only advances the cursor, and k_nbr_finish turns cursor > capacity into the
  * overflow state (nbr_len = -1, TS_FLAG_NBR_OVERFLOW).  The grid is capped (grid-stride over the slots): when no
@@ -243,6 +244,15 @@ __global__ void __launch_bounds__(256) k_nbr_fill(DevState d)
         const int c2 = lin % nb2, c1 = (lin / nb2) % nb1, c0 = lin / (nb2 * nb1);
         const int D0 = g.D[0], D1 = g.D[1], D2 = g.D[2];
         int cnt = 0;
+        long long start = 0;
+        const long long seg = d.nbr_base[s], cap = d.nbr_base[s + 1] - seg;
+        /* pass 0 buffers the row in shared memory; a row longer than the buffer is walked a second time and written
+         * straight into its reserved place (pass 1: rare, so the second walk costs nothing on average) */
+        for (int pass = 0; pass < 2; ++pass) {
+        const bool direct = pass == 1;
+        unsigned *const out = d.nbr + seg + start;
+        const bool room = start + cnt <= cap;                    /* pass 1: cnt is the length found by pass 0 */
+        cnt = 0;
         for (int e0 = c0 - D0; e0 <= c0 + D0; ++e0) {
             const int s0 = floordiv(e0, nb0), b0 = e0 - s0 * nb0;
             for (int e1 = c1 - D1; e1 <= c1 + D1; ++e1) {
@@ -270,23 +280,26 @@ __global__ void __launch_bounds__(256) k_nbr_fill(DevState d)
                         }
                         const unsigned m = (__ballot_sync(qmask, ok) >> (8 * qg)) & 0xffu;
                         const int at = cnt + __popc(m & lt);
-                        if (ok && at < NBR_BUF) mybuf[at] = ts_pack_nbr(lj, s0, s1, s2);
+                        if (ok) {
+                            if (direct) { if (room) out[at] = ts_pack_nbr(lj, s0, s1, s2); }
+                            else if (at < NBR_BUF) mybuf[at] = ts_pack_nbr(lj, s0, s1, s2);
+                        }
                         cnt += __popc(m);
                     }
                 }
             }
         }
+        if (direct) break;
         /* reserve the row and copy it out */
-        long long start = 0;
-        if (l == 0) {
-            const unsigned long long want = cnt <= NBR_BUF ? (unsigned long long)cnt : (1ull << 40);   /* too long for the buffer: overflow */
-            start = (long long)atomicAdd((unsigned long long *)&d.nbr_len[s], want);
-        }
+        if (l == 0) start = (long long)atomicAdd((unsigned long long *)&d.nbr_len[s], (unsigned long long)cnt);
         start = __shfl_sync(qmask, start, 8 * qg);
-        const long long seg = d.nbr_base[s], cap = d.nbr_base[s + 1] - seg;
         __syncwarp(qmask);
-        if (cnt <= NBR_BUF && start + cnt <= cap)
-            for (int k = l; k < cnt; k += 8) d.nbr[seg + start + k] = mybuf[k];
+        if (cnt <= NBR_BUF) {
+            if (start + cnt <= cap)
+                for (int k = l; k < cnt; k += 8) d.nbr[seg + start + k] = mybuf[k];
+            break;
+        }
+        }
         __syncwarp(qmask);
         if (l == 0) {
             d.nbr_off[a0 + li] = seg + start;
@@ -349,5 +362,5 @@ void launch_build(ts_state *st, bool force, cudaStream_t q)
     k_nbr_finish<<<(d.S + 255) / 256, 256, 0, q>>>(d);
     k_build_end<<<(d.S + 255) / 256, 256, 0, q>>>(d);
     st->launches += 7;
-    st->list_built = true;
+    if (force) st->list_built = true;                          /* a skin-checked build keeps what the forced one established */
 }

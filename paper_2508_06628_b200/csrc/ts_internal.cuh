@@ -105,6 +105,8 @@ struct ts_state {
     ts_state_desc desc;
     ts_nbr_params nbr;
     int *h_sysoff;               /* host copy [S+1]                    */
+    long long N_cap;             /* atoms / systems the state was created with: the capacity ts_repack_systems fills */
+    int S_cap;
     bool list_built;             /* a build has been enqueued and no swap since */
     bool forces_current;
     int engine;
@@ -136,6 +138,8 @@ TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types
     } while (0)
 void ts_set_error(ts_state *st, const char *fmt, ...);
 
+/* ts_api.cu */
+long long ts_system_pair_capacity(long long n, double vol, double r_list, double slack);
 /* ts_build.cu */
 void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, cudaStream_t q);
 void launch_build(ts_state *st, bool force, cudaStream_t q);

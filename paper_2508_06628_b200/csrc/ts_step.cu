@@ -81,7 +81,7 @@ extern "C" ts_status ts_md_step(ts_state *st, const ts_md_params *p, int32_t n_s
         }
     }
     st->last_engine = 0;
-    if (!st->forces_current || n_steps == 0) {
+    if (!st->forces_current || !st->list_built || n_steps == 0) {   /* no list of its own yet (e.g. the resident engine ran before) */
         ensure_list(st, q);
         launch_pair(st, n_steps == 0 ? want : 0u, false, q);
         if (n_steps == 0) launch_kinetic(st, q);

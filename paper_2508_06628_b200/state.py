@@ -43,6 +43,8 @@ class SimState:
         self.npdtype = np.float32 if self.dtype == ts.TS_F32 else np.float64
         self.N = int(np.asarray(batch.pos).shape[0])
         self.S = int(np.asarray(batch.cell).shape[0])
+        self.N_cap, self.S_cap = self.N, self.S                 # what ts_repack_systems may fill (sizes at create)
+        self.sys_offset = np.asarray(batch.sys_offset, dtype=np.int64).copy() if hasattr(batch, "sys_offset") else None
         self.skin = float(batch.skin if skin is None else skin)
         self.slack = float(slack)
         self.units = ts.ts_units(float(batch.mass_conv), float(batch.kB))
@@ -138,23 +140,84 @@ class SimState:
 
     def swap_systems(self, slots, fresh):
         """Replace the systems in `slots` by those of `fresh` (duck-typed batch, same sizes)."""
+        d, alive = self._upload_fresh(fresh)
+        ts.ts_swap_systems(self.handle, slots, d)   # synchronises: the uploads may be released afterwards
+        del alive
+
+    def _upload_fresh(self, fresh):
+        """Device copies of a duck-typed batch for a swap / repack and their descriptor (kept alive by the caller)."""
         torch = self.torch
-        n = len(slots)
+        n = int(np.asarray(fresh.cell).shape[0])
         nat = int(np.asarray(fresh.pos).shape[0])
         dev = self.device
 
         def up(a, dt, shape):
             return torch.from_numpy(np.ascontiguousarray(np.asarray(a).reshape(shape))).to(dt).to(dev).contiguous()
 
-        keep = [up(fresh.pos, self.tdtype, (nat, 3)), up(fresh.vel, self.tdtype, (nat, 3)),
+        vel = fresh.vel if getattr(fresh, "vel", None) is not None else np.zeros((nat, 3))
+        keep = [up(fresh.pos, self.tdtype, (nat, 3)), up(vel, self.tdtype, (nat, 3)),
                 up(fresh.mass, self.tdtype, (nat,)), up(fresh.type, torch.int32, (nat,)),
                 up(fresh.cell, self.tdtype, (n, 3, 3)),
                 torch.from_numpy(np.asarray(fresh.sys_uid).astype(np.int64)).to(torch.int32).to(dev)]
         p = lambda t: C.c_void_p(t.data_ptr())
         d = ts.ts_state_desc(nat, n, self.dtype, self.units, p(keep[0]), p(keep[1]), None, p(keep[2]), p(keep[3]),
                              None, p(keep[4]), None, None, None, p(keep[5]))
-        ts.ts_swap_systems(self.handle, slots, d)   # synchronises: `keep` may be released afterwards
+        return d, keep
+
+    def repack(self, keep_slots, fresh=None):
+        """Ragged in-flight replacement (ts_repack_systems): the batch becomes the kept slots, in order, followed by
+        the systems of `fresh` (duck-typed batch, any sizes).  Raises TsError(WORKSPACE_TOO_SMALL) when the new batch
+        does not fit the capacity of the state; nothing has changed then."""
+        keep_slots = [int(k) for k in keep_slots]
+        old = self.sys_offset
+        sizes = [int(old[k + 1] - old[k]) for k in keep_slots]
+        if fresh is not None:
+            d, alive = self._upload_fresh(fresh)
+            fn = np.diff(np.asarray(fresh.sys_offset)).astype(np.int32)
+            ts.ts_repack_systems(self.handle, keep_slots, d, fn)
+            sizes += [int(x) for x in fn]
+            del alive
+        else:
+            ts.ts_repack_systems(self.handle, keep_slots, None, np.zeros(0, np.int32))
+        self.sys_offset = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+        self.N, self.S = int(self.sys_offset[-1]), len(sizes)
+
+    def capacity(self):
+        """(atoms, systems, pair slots) the state was created with."""
+        return ts.ts_get_capacity(self.handle)
+
+    # ------------------------------------------------------------------ graph export / external model (NEXT-2)
+    def export_edges(self, cap=None):
+        """The current Verlet list as device tensors: edge_index [2, n_edges] (int64) and the integer image shifts
+        [n_edges, 3] in the state dtype: r_ij = pos[j] - pos[i] + shift @ cell[system].  Reads one scalar back
+        (the edge count) to slice the tensors."""
+        torch = self.torch
+        if cap is None:
+            cap = self.capacity()[2]
+        if getattr(self, "_edges", None) is None or self._edges[0].shape[1] < cap:
+            self._edges = (torch.empty((2, cap), dtype=torch.int64, device=self.device),
+                           torch.empty((cap, 3), dtype=self.tdtype, device=self.device),
+                           torch.zeros(1, dtype=torch.int64, device=self.device))
+        ei, es, ne = self._edges
+        ts.ts_export_edges(self.handle, ei[0].data_ptr(), ei[1].data_ptr(), es.data_ptr(), ei.shape[1], ne.data_ptr())
+        n = int(ne.item())
+        if n > ei.shape[1]:
+            raise ts.TsError(ts.TS_ERR_WORKSPACE_TOO_SMALL, "export_edges", f"{n} edges > capacity {ei.shape[1]}")
+        return ei[:, :n], es[:n]
+
+    def md_step_external(self, params, phase):
+        if isinstance(params, dict):
+            params = ts.md_params(**params)
+        ts.ts_md_step_external(self.handle, params, phase)
+
+    def fire_step_external(self, params, phase):
+        if isinstance(params, dict):
+            params = ts.fire_params(**params)
+        ts.ts_fire_step_external(self.handle, params, phase)
 
     # ------------------------------------------------------------------ host views
     def numpy(self, name):
-        return getattr(self, name).detach().cpu().numpy()
+        """Host copy of a boundary array, cut to the live batch (a repack may have shrunk it below the capacity)."""
+        t = getattr(self, name)
+        n = self.S if name in ("cell", "energy", "virial", "kinetic", "sys_uid") else self.N
+        return t[:n].detach().cpu().numpy()

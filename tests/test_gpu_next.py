@@ -1,0 +1,177 @@
+"""GPU tests of the rows SURVEY.md 8(f) calls "next" and of the ragged in-flight path of row a10:
+ts_repack_systems / RaggedInFlightRelaxer (K12), BinRunner (NEXT-1),
+ts_export_edges + external-model stepping (NEXT-2).  Every comparison is with the fp64 CPU
+oracle of the system run alone (O7: systems are independent, so batch composition must not matter)."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ts():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2508_06628_b200 as m
+    m.lib()
+    return m
+
+
+SIZES = [48, 96, 64, 160, 80, 128, 56, 112, 72, 144, 40, 104]     # atoms of stream id k: SIZES[k % 12]
+
+
+def _mixed(sid):
+    """Stream id -> one soft-sphere system whose size depends on the id (Fig. 3: structures of different sizes)."""
+    return wl.cfg4([sid], n_atoms=SIZES[sid % len(SIZES)])
+
+
+@pytest.mark.parametrize("engine", [0, 1])
+def test_repack_keeps_running_systems_and_admits_fresh_ones(ts, orc, engine):
+    """ts_repack_systems in the middle of a FIRE run: the kept systems continue exactly as if nothing had happened
+    (state after 60 steps equals the oracle's solo run to 1e-8), the fresh ones start at step 0."""
+    ids = [0, 1, 2, 3]
+    b = wl.concat([_mixed(i) for i in ids])
+    fire = dict(b.fire, f_max=1e-30, max_steps=10 ** 6)       # nobody converges: compare raw trajectories
+    st = ts.SimState(b, engine=engine)
+    st.fire_step(fire, 25)
+    fresh = wl.concat([_mixed(7), _mixed(10)])                # 112 + 40 atoms into the room of systems 1 (96) and 3 (160)
+    st.repack([2, 0], fresh)                                  # kept in a NEW order: old 2, old 0, then 7, 10
+    assert (st.N, st.S) == (64 + 48 + 112 + 40, 4)
+    st.fire_step(fire, 35)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == engine
+    pos, steps = st.numpy("pos"), st.converged_mask()[2]
+    assert list(steps) == [60, 60, 35, 35]
+    off = st.sys_offset
+    for k, (sid, n) in enumerate([(2, 60), (0, 60), (7, 35), (10, 35)]):
+        one = _mixed(sid)
+        o = orc.fire_run(one, dict(one.fire, f_max=1e-30, max_steps=10 ** 6), n)
+        assert np.abs(pos[off[k]:off[k + 1]] - o["pos"]).max() <= 1e-8, (sid, n)
+    # capacity: a batch that does not fit is refused and nothing changes
+    with pytest.raises(ts.TsError) as err:
+        st.repack([0, 1, 2, 3], wl.concat([_mixed(3), _mixed(9)]))
+    assert err.value.code == ts.TS_ERR_WORKSPACE_TOO_SMALL and (st.N, st.S) == (264, 4)
+    st.fire_step(fire, 5)
+    assert st.poll().flags == 0 and list(st.converged_mask()[2]) == [65, 65, 40, 40]
+    st.close()
+
+
+def test_ragged_inflight_relaxer_mixed_sizes(ts, orc):
+    """A stream of systems of different sizes through one state with a byte budget: every id is relaxed exactly once,
+    the capacity is never exceeded, every final state passes the oracle's own convergence check, and the results do
+    not depend on the budget or the check cadence (R22)."""
+    from paper_2508_06628_b200 import scheduler as sch
+    n_total = 14
+    fire = dict(_mixed(0).fire, f_max=1e-4, max_steps=20000)
+    per = [sch.batch_system_bytes(_mixed(i))[0] for i in range(n_total)]
+    r = sch.RaggedInFlightRelaxer(_mixed, n_total, fire, budget_bytes=sum(per[:4]) + 1.0, k_check=10)
+    res = r.run()
+    assert sorted(res) == list(range(n_total)) and r.unfinished == [] and r.failed == []
+    assert r.n_repacks >= 3 and r.peak_systems <= 4 and r.peak_atoms <= sum(SIZES[:4])
+    for sid, rec in res.items():
+        assert rec["status"] == ts.TS_FIRE_CONVERGED and rec["pos"].shape[0] == SIZES[sid % len(SIZES)]
+        o = orc.energy_forces(wl.with_(_mixed(sid), pos=rec["pos"]))
+        assert np.sqrt((o["F"] ** 2).sum(1)).max() < fire["f_max"]             # R30(ii)
+        assert abs(rec["energy"] - o["E"][0]) <= 1e-12 * max(abs(o["E"][0]), o["Eabs"][0])
+    r2 = sch.RaggedInFlightRelaxer(_mixed, n_total, fire, budget_bytes=sum(per[:6]) + 1.0, k_check=7)
+    res2 = r2.run()
+    for sid in res:
+        assert res2[sid]["fire_steps"] == res[sid]["fire_steps"]
+        assert np.abs(res2[sid]["pos"] - res[sid]["pos"]).max() <= 1e-6
+
+
+def test_bin_runner_matches_solo_runs(ts, orc):
+    """BinningAutobatcher as a runner: a ragged Morse batch packed into bins by the byte scaler and stepped bin by bin
+    on two streams; every system's trajectory equals the oracle run of that system alone."""
+    from paper_2508_06628_b200 import scheduler as sch
+    b = wl.cfg3(n_systems=9, dtype="f64", n_range=(32, 300))
+    costs = sch.batch_system_bytes(b)
+    runner = sch.BinRunner(b, budget_bytes=1.05 * max(costs.max(), costs.sum() / 4))
+    assert len(runner.bins) >= 3 and sorted(np.concatenate(runner.bins).tolist()) == list(range(9))
+    for systems in runner.bins:
+        assert costs[systems].sum() <= runner_budget(runner, costs)
+    out = runner.run_md(40, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    o = orc.md_run(b, "nve", b.md["dt"], 40)
+    assert np.abs(out["pos"] - o["pos"]).max() <= 1e-8
+    assert np.allclose(out["energy"], o["E"], rtol=1e-10) and np.allclose(out["kinetic"], o["KE"], rtol=1e-10)
+
+
+def runner_budget(runner, costs):
+    return 1.05 * max(costs.max(), costs.sum() / 4)
+
+
+def _torch_lj_forces(torch, pos, cell, system_idx, edge_index, shift, eps, sigma, rc):
+    """The stand-in external model: Lennard-Jones forces from the exported edge list in plain torch ops."""
+    i, j = edge_index[0], edge_index[1]
+    h = cell[system_idx[i].long()]                                           # [E,3,3], rows = lattice vectors
+    rij = pos[j] - pos[i] + torch.einsum("ek,ekc->ec", shift, h)
+    r2 = (rij * rij).sum(1)
+    inside = r2 < rc * rc
+    s6 = (sigma * sigma / r2) ** 3
+    g = torch.where(inside, -24.0 * eps * (2.0 * s6 * s6 - s6) / r2, torch.zeros_like(r2))   # V'(r) / r
+    F = torch.zeros_like(pos)
+    F.index_add_(0, i, g[:, None] * rij)                                     # F_i = sum V'(r) r_ij / r
+    return F
+
+
+def test_edge_export_and_external_model_md(ts, orc):
+    """NEXT-2: the list exported on the device is the oracle's pair set at r_list; an external force provider (plain
+    torch on the GPU) driven through ts_md_step_external reproduces the oracle's NVE trajectory."""
+    import torch
+    b = wl.cfg1(n_systems=3, reps=3)                           # 3 x 108 atoms, box 15.78 A < 2 r_list: image shifts matter
+    st = ts.SimState(b, engine=0)
+    md = ts.md_params(**b.md)
+    st.md_step_external(md, ts.TS_PHASE_INIT)
+    ei, es = st.export_edges()
+    got = set(zip(ei[0].tolist(), ei[1].tolist(), *[es[:, k].to(torch.int64).tolist() for k in range(3)]))
+    want = set()
+    for s in range(b.n_systems):
+        a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+        i, j, S, _ = orc.pairs(b.pos[a0:a1], b.cell[s], b.r_list)
+        want |= set(zip((i + a0).tolist(), (j + a0).tolist(), S[:, 0].tolist(), S[:, 1].tolist(), S[:, 2].tolist()))
+    assert got == want and len(got) == ei.shape[1]
+    pot = b.potential
+    eps, sigma, rc = float(pot.p0[0, 0]), float(pot.p1[0, 0]), float(pot.rc[0, 0])
+    model = lambda: _torch_lj_forces(torch, st.pos, st.cell, st.system_idx, *st.export_edges(), eps, sigma, rc)
+    st.force.copy_(model())
+    n = 25
+    for _ in range(n):
+        st.md_step_external(md, ts.TS_PHASE_PRE)
+        st.force.copy_(model())
+        st.md_step_external(md, ts.TS_PHASE_POST)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.steps_done == n
+    o = orc.md_run(b, "nve", b.md["dt"], n)
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
+    assert np.allclose(st.numpy("kinetic"), o["KE"], rtol=1e-10)
+    assert np.array_equal(st.get_system_steps(), np.full(3, n, np.uint64))
+    st.close()
+
+
+def test_external_model_fire_matches_library_fire(ts, orc):
+    """FIRE driven through ts_fire_step_external with the library's own pair kernel as the "external" provider gives the
+    state of ts_fire_step (to rounding: the energy-only and the full pair kernel sum in different orders), and both
+    follow the oracle for the first 60 steps."""
+    b = wl.cfg4(range(3), n_atoms=64)
+    fire = dict(b.fire, f_max=1e-30, max_steps=10 ** 6)
+    ref = ts.SimState(b, engine=0)
+    ref.fire_step(fire, 60)
+    st = ts.SimState(b, engine=0)
+    fp = ts.fire_params(**fire)
+    st.fire_step_external(fp, ts.TS_PHASE_INIT)
+    st.compute_forces(ts.TS_WANT_ENERGY)
+    st.fire_step_external(fp, ts.TS_PHASE_CHECK0)
+    for _ in range(60):
+        st.fire_step_external(fp, ts.TS_PHASE_PRE)
+        st.compute_forces(ts.TS_WANT_ENERGY)
+        st.fire_step_external(fp, ts.TS_PHASE_POST)
+    assert st.poll().flags == 0
+    assert np.abs(st.numpy("pos") - ref.numpy("pos")).max() <= 1e-10 and np.abs(st.numpy("vel") - ref.numpy("vel")).max() <= 1e-10
+    o = orc.fire_run(b, fire, 60)
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert list(st.converged_mask()[2]) == [60, 60, 60]
+    st.close(); ref.close()

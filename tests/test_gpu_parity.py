@@ -246,3 +246,45 @@ def test_resident_engine_is_deterministic(ts):
         st.close()
     for a, c in zip(*outs):
         assert np.array_equal(a, c)
+
+
+def test_rows_longer_than_the_build_buffer(ts, orc):
+    """General engine: a list radius with more than 256 neighbours per atom (the shared-memory row buffer of the
+    one-pass neighbour search): the long rows take the second walk; pair sets stay bit-exact, E / F / W in tolerance."""
+    b = wl.cfg1(n_systems=2, reps=4)
+    st = ts.SimState(b, skin=6.0, engine=0)                    # r_list = 14.5 A: ~350 neighbours per atom
+    st.compute_forces(ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    off, j, shift = st.get_neighbors()
+    rep = st.poll()
+    assert rep.flags == 0 and rep.list_valid == 1 and rep.max_neighbors > 256
+    i = np.repeat(np.arange(b.n_atoms), np.diff(off))
+    got = set(zip(i.tolist(), j.tolist(), shift[:, 0].tolist(), shift[:, 1].tolist(), shift[:, 2].tolist()))
+    want = set().union(*_pair_sets(orc, b, b.potential.rc_max + 6.0))
+    assert got == want and len(got) == j.size
+    _check_efw(b, st, orc.energy_forces(b), False)
+    st.close()
+
+
+RESIDENT_STATIC = {
+    "cfg1_f64": lambda: wl.cfg1(n_systems=4),
+    "cfg2_f32": lambda: wl.cfg2(n_systems=3, dtype="f32"),
+    "cfg2_f64": lambda: wl.cfg2(n_systems=2, dtype="f64"),
+    "cfg3_f32": lambda: wl.cfg3(n_systems=6, dtype="f32", n_range=(500, 900)),
+    "cfg3_f64": lambda: wl.cfg3(n_systems=4, dtype="f64", n_range=(500, 700)),
+    "cfg4_f64": lambda: wl.cfg4(range(6)),
+    "cfg4_f32": lambda: wl.cfg4(range(4), dtype="f32"),
+}
+
+
+@pytest.mark.parametrize("name", list(RESIDENT_STATIC))
+def test_resident_engine_static_energy_forces_virial(ts, orc, name):
+    """The pair phase of the system-resident engine at step 0 (no integration): E, F and the 3x3 virial of LJ, Morse
+    and the two-type soft-sphere table against the oracle, fp32 and fp64, element by element."""
+    b = RESIDENT_STATIC[name]()
+    o = orc.energy_forces(b)
+    st = ts.SimState(b, engine=1)
+    st.md_step(dict(b.md) if b.md else dict(integrator="nve", dt=1.0), 0, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 1, (rep.flags, rep.engine)
+    _check_efw(b, st, o, b.dtype == "f32")
+    st.close()

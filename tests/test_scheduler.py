@@ -122,3 +122,71 @@ def test_world_size_2_gloo_sharding(tmp_path):
     for r, p in enumerate(procs):
         out, _ = p.communicate(timeout=240)
         assert p.returncode == 0 and f"ok {r}" in out, out
+
+
+def test_take_and_concat_are_pure_container_work():
+    import workloads as wl
+    b = wl.cfg3(n_systems=5, dtype="f64", n_range=(32, 120), clean=False)
+    t = sch.take_systems(b, [3, 1])
+    ref = wl.take(b, [3, 1])
+    for name in ("pos", "vel", "mass", "type", "system_idx", "sys_offset", "cell", "sys_uid"):
+        assert np.array_equal(np.asarray(getattr(t, name)), np.asarray(getattr(ref, name))), name
+    c = sch.concat_systems([sch.take_systems(b, [0]), t])
+    assert c.n_systems == 3 and c.n_atoms == int(np.diff(b.sys_offset)[[0, 3, 1]].sum())
+    assert np.array_equal(c.pos[c.sys_offset[1]:c.sys_offset[2]], b.pos[b.sys_offset[3]:b.sys_offset[4]])
+
+
+_SHARD_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch, torch.distributed as dist
+import workloads as wl
+from paper_2508_06628_b200 import scheduler as sch
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+store = dist.TCPStore("127.0.0.1", int(os.environ["STORE_PORT"]), world, rank == 0)
+dist.init_process_group("gloo", store=store, rank=rank, world_size=world)
+b = wl.cfg3(n_systems=9, dtype="f64", n_range=(32, 200), clean=False)
+runner = sch.ShardedRunner(store=store)
+# fixed-length mode: every rank "steps" its shard with a stand-in (the real step_fn is a SimState run: no CPU path
+# exists, by design); the gather must return every system exactly once, with the data of the right system
+def step_fn(sub, systems):
+    assert sub.n_systems == len(systems)
+    return {{s: (rank, float(sub.pos[sub.sys_offset[k]:sub.sys_offset[k + 1]].sum())) for k, s in enumerate(systems)}}
+res = runner.run_fixed(b, step_fn)
+mine, load = runner.shard(sch.batch_system_bytes(b))
+assert load.max() <= 1.34 * load.sum() / world + sch.batch_system_bytes(b).max()
+if rank == 0:
+    assert sorted(res) == list(range(9))
+    for s, (r, v) in res.items():
+        assert abs(v - float(b.pos[b.sys_offset[s]:b.sys_offset[s + 1]].sum())) < 1e-9
+    assert {{r for r, _ in res.values()}} == {{0, 1}}
+else:
+    assert res is None
+# in-flight mode: one shared counter hands out stream ids; ranks claim different amounts, nothing is lost or doubled
+claimed = []
+while True:
+    ids = runner.next_ids(1 + rank * 2, 23)
+    if not ids and len(claimed) and claimed[-1] >= 0:
+        pass
+    if not ids:
+        break
+    claimed += ids
+every = [None] * world
+dist.all_gather_object(every, claimed)
+flat = sorted(i for part in every for i in part)
+assert flat == list(range(23)), flat
+dist.barrier(); dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_sharded_runner_world_size_2_gloo(tmp_path):
+    script = tmp_path / "s.py"
+    script.write_text(_SHARD_WORKER.format(root=ROOT))
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT="29573", STORE_PORT="29575")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+    for r, p in enumerate(procs):
+        out, _ = p.communicate(timeout=240)
+        assert p.returncode == 0 and f"ok {r}" in out, out
