@@ -27,8 +27,22 @@ sys.path.insert(0, ROOT)
 
 import workloads as wl  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per k_resident_md launch (1000 MD steps), profiles/r01_ncu_resident_cfg2_fp32.md
-NCU_TRAFFIC = {"resident": 1.895936e6 + 1280.0, "general": None}
+TRAFFIC_PROFILE = os.path.join(ROOT, "profiles", "r02_ncu_resident_cfg2_fp32.md")
+
+
+def profile_traffic(path=TRAFFIC_PROFILE):
+    """dram__bytes_read.sum + dram__bytes_write.sum per k_resident_md launch (one bench step), read from the tracked ncu
+    summary of this command (a markdown table row per metric: | `name` | unit | value |); None if the file is absent."""
+    if not os.path.exists(path):
+        return None, None
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot, seen = 0.0, 0
+    for line in open(path):
+        f = [x.strip().strip("`") for x in line.strip().strip("|").split("|")]
+        if len(f) == 3 and f[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and f[1] in scale:
+            tot += float(f[2]) * scale[f[1]]
+            seen += 1
+    return (tot if seen == 2 else None), os.path.relpath(path, ROOT)
 
 METRIC = "atom_steps_per_s"
 UNIT = "atom-steps/s"
@@ -105,13 +119,24 @@ def max_over_ranks(times, world, device):
     return [float(x) for x in t]
 
 
-def algorithmic_model(nbar, K, w=4, entry_bytes=4):
+PAIR_FLOPS = {"lj": 32.0, "morse": 40.0, "soft_sphere": 28.0}
+
+
+def algorithmic_model(nbar, K, w=4, entry_bytes=4, kind="lj", virial=False):
     """bytes and FLOPs one atom-step must move / do with a directed Verlet list."""
     state = 2 * 3 * w + 3 * 3 * w + w + 4
     lst = entry_bytes * nbar
     rebuild = (2 * 3 * w + 8 + lst) / max(K, 1.0)
-    flops = 32.0 * nbar + 20.0
+    flops = (PAIR_FLOPS[kind] + (12.0 if virial else 0.0)) * nbar + 20.0
     return state + lst + rebuild, flops
+
+
+def fma_peaks(device):
+    """Measured register-only FMA rates (ts_measure_fma_tflops): fp32 FFMA, fp64 DFMA, packed fp32 FFMA2, in TFLOP/s."""
+    import torch
+    import paper_2508_06628_b200 as ts
+    scratch = torch.zeros(4096, dtype=torch.uint8, device=device)
+    return {k: ts.ts_measure_fma_tflops(i, scratch.data_ptr()) for i, k in enumerate(("fp32", "fp64", "fp32x2"))}
 
 
 def run_reference(args):
@@ -130,7 +155,8 @@ def run_reference(args):
         oracle.md_run(b, "baoab", md["dt"], md_steps, temperature=md["temperature"], friction=md["friction"],
                       seed=md["seed"], sys_uid=b.sys_uid, nthreads=cores)
 
-    for _ in range(max(args.warmup, 1) if args.warmup < 2 else 1):
+    n_warm = 1                                                 # one untimed call (the oracle has no state to warm; each call is seconds)
+    for _ in range(n_warm):
         step()
     t0 = time.perf_counter()
     for _ in range(args.steps):
@@ -140,7 +166,7 @@ def run_reference(args):
     sample = f"{n_sys} of 64 systems x 864 atoms, {md_steps} BAOAB steps (+1 initial force pass) per bench step, fp64 O(N^2) all-images"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": n_warm, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "cfg2: 64x864 FCC Ar LJ, BAOAB 80K (BASELINE.json:configs[1])", "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -163,24 +189,38 @@ def cpu_baseline():
                       f"{dt:.1f} s wall on {cores} threads"}
 
 
-def run_secondary(args):
-    """The other BASELINE.json configs at full size, device-timed (CUDA events, inputs resident, rebuilds inside): context
-    for BASELINE.md section 5, not the graded line.  A step = one ts_md_step / ts_fire_step call of `inner` steps."""
+YARDSTICK = {  # SURVEY.md 8(d) "Yardstick values": which potential / virial the byte and FLOP model of a config uses
+    "cfg1": ("lj", False), "cfg2_f64": ("lj", False), "cfg3": ("morse", True), "cfg4": ("soft_sphere", False),
+    "cfg4_general": ("soft_sphere", False), "cfg5": ("lj", False),
+}
+
+
+def secondary_line(w, steps, warmup, engine=1, systems=None, hbm_budget_gb=150.0, peaks=None, hbm_peak=None):
+    """One of the other BASELINE.json configs at full size, device-timed (CUDA events, inputs resident, rebuilds inside):
+    a dict with the metric, the measured n-bar and K, and its own SURVEY 8(d) roofline.  A step = one ts_md_step /
+    ts_fire_step call of `inner` steps."""
     import torch
     import paper_2508_06628_b200 as ts
-    ts.lib()
-    w = args.workload
-    fire = False
+    from paper_2508_06628_b200 import scheduler as sch
+    fire, extra = False, {}
     if w == "cfg1":
         b, inner = wl.cfg1(n_systems=4), 100
     elif w == "cfg2_f64":
         b, inner = wl.cfg2(n_systems=64, dtype="f64"), 200
     elif w == "cfg3":
         b, inner = wl.cfg3(n_systems=512, dtype="f32"), 100
-    elif w == "cfg4":
+    elif w in ("cfg4", "cfg4_general"):
         b, inner, fire = wl.cfg4(range(1024)), 100, True
+        engine = 0 if w == "cfg4_general" else engine
     elif w == "cfg5":
-        start = wl.cfg5_start(range(args.systems if args.systems != 64 else 10000))
+        # batch size chosen by the memory estimator for a stated HBM budget (BASELINE.json configs[4]; PAPER.md:66, :88)
+        probe = wl.cfg5_start(range(1))
+        per = float(sch.batch_system_bytes(probe)[0])
+        want = 10000 if systems is None else int(systems)
+        n_fit = sch.admit(np.full(want, per), hbm_budget_gb * 1e9)
+        extra = {"estimator": {"bytes_per_system": per, "hbm_budget_gb": hbm_budget_gb, "systems_admitted": int(n_fit),
+                               "systems_asked": want, "batches": int(np.ceil(want / max(n_fit, 1)))}}
+        start = wl.cfg5_start(range(n_fit))
         sf = ts.SimState(start)
         sf.fire_step(dict(start.fire, f_max=1e-12, max_steps=10**6), 200)      # R33: pre-relaxation by the library itself
         relaxed = wl.with_(start, pos=sf.numpy("pos").astype(np.float64))
@@ -188,32 +228,93 @@ def run_secondary(args):
         b, inner = wl.cfg5_md(relaxed), 200
     else:
         raise SystemExit(f"unknown workload {w}")
-    st = ts.SimState(b, engine=args.engine)
+    st = ts.SimState(b, engine=engine)
     if fire:
         params = dict(b.fire, f_max=1e-30)                     # nobody converges: every step does the full work
         call = lambda: st.fire_step(params, inner)
     else:
-        want = ts.TS_WANT_ENERGY | (ts.TS_WANT_VIRIAL if w == "cfg3" else 0)
-        call = lambda: st.md_step(dict(b.md), inner, want)
-    for _ in range(max(args.warmup, 3)):
+        want_flags = ts.TS_WANT_ENERGY | (ts.TS_WANT_VIRIAL if w == "cfg3" else 0)
+        call = lambda: st.md_step(dict(b.md), inner, want_flags)
+    warm = max(warmup, 3)
+    for _ in range(warm):
         call()
+    rep0 = st.poll()
+    clocks = ClockSampler(torch.cuda.current_device())
     torch.cuda.synchronize()
+    clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         call()
     e1.record()
     torch.cuda.synchronize()
+    clk = clocks.stop()
     rep = st.poll()
-    ms = e0.elapsed_time(e1) / args.steps
-    print(json.dumps({"metric": METRIC, "value": b.n_atoms * inner / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
-                      "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
-                      "dtype": b.dtype, "secondary": True,
-                      "config": {"workload": w, "systems": b.n_systems, "atoms": b.n_atoms, "steps_per_call": inner,
-                                 "kind": "fire" if fire else b.md.get("integrator"), "us_per_inner_step": ms * 1e3 / inner,
-                                 "engine": "resident" if rep.engine == 1 else "general", "flags": int(rep.flags),
-                                 "mean_neighbours": rep.nnz / b.n_atoms}}))
+    ms = e0.elapsed_time(e1) / steps
+    nbar = rep.nnz / b.n_atoms
+    K = steps * inner * b.n_systems / max(rep.resident_rebuilds - rep0.resident_rebuilds, 1)
+    wbytes = 4 if b.dtype == "f32" else 8
+    kind, virial = YARDSTICK.get(w, ("lj", False))
+    b_alg, flops = algorithmic_model(nbar, K, wbytes, 4, kind, virial)
+    value = b.n_atoms * inner / (ms * 1e-3)
+    if hbm_peak is None:
+        hbm_peak = measured_peaks()[0]
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warm, "ms_per_step": ms,
+            "higher_is_better": True, "data": "synthetic", "dtype": b.dtype, "secondary": True,
+            "config": dict({"workload": w, "systems": b.n_systems, "atoms": b.n_atoms, "steps_per_call": inner,
+                            "kind": "fire" if fire else b.md.get("integrator"), "us_per_inner_step": ms * 1e3 / inner,
+                            "engine": "resident" if rep.engine == 1 else "general", "flags": int(rep.flags),
+                            "mean_neighbours": nbar, "steps_per_rebuild": K}, **extra),
+            "clocks": clk,
+            "roofline": {"bound": "hbm", "achieved": b_alg * value / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": b_alg * value / 1e9 / hbm_peak, "traffic": None,
+                         "model": f"B_alg = {b_alg:.1f} B/atom-step (SURVEY 8(d): state + 4 B x nbar {nbar:.1f} + rebuild / K, K = {K:.1f})",
+                         "alu": {"flop_per_atom_step": flops, "achieved_tflops": flops * value / 1e12,
+                                 "peak_tflops": None if peaks is None else peaks["fp32" if b.dtype == "f32" else "fp64"],
+                                 "peak_source": "measured: ts_measure_fma_tflops (register-only FMA chains)"}}}
     st.close()
+    return line
+
+
+def run_cfg4_inflight(args):
+    """BASELINE.json configs[3] as stated: 1024 slots, converged systems swapped out for fresh seeded ones until 4096 are
+    relaxed (R24).  Wall time of the whole in-flight run (host scheduling and swaps included), failed ids listed."""
+    import torch
+    import paper_2508_06628_b200 as ts
+    from paper_2508_06628_b200 import scheduler as sch
+    n_target, n_slots = int(args.target), 1024
+    make = lambda ids: wl.cfg4(ids)
+    fire = dict(make([0]).fire)
+    r = sch.InFlightRelaxer(make, n_total=n_target + 2 * n_slots, fire=fire, n_slots=n_slots, k_check=args.k_check, engine=args.engine)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = r.run(target=n_target)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    conv = [i for i, x in res.items() if x["status"] == ts.TS_FIRE_CONVERGED]
+    steps = np.array([res[i]["fire_steps"] for i in conv])
+    total_steps = int(sum(x["fire_steps"] for x in res.values()))
+    print(json.dumps({"metric": "systems_relaxed_per_s", "value": len(conv) / dt, "unit": "systems/s", "n_gpus": 1,
+                      "higher_is_better": True, "data": "synthetic", "dtype": "f64", "secondary": True,
+                      "config": {"workload": "cfg4_inflight: 1024 slots x 256 atoms, FIRE to max|F| < 1e-4, swap until relaxed",
+                                 "relaxed": len(conv), "target": n_target, "failed_ids": sorted(r.failed),
+                                 "unfinished_in_slots": len(r.unfinished), "k_check": args.k_check,
+                                 "engine": "resident" if args.engine == 1 else "general",
+                                 "fire_steps_median": float(np.median(steps)), "fire_steps_max": int(steps.max()),
+                                 "wall_s": dt, "atom_steps_per_s": 256.0 * total_steps / dt}}))
+    return 0
+
+
+def run_secondary(args):
+    if args.workload == "cfg4_inflight":
+        return run_cfg4_inflight(args)
+    import torch
+    import paper_2508_06628_b200 as ts
+    ts.lib()
+    peaks = fma_peaks(torch.device("cuda", 0))
+    line = secondary_line(args.workload, args.steps, args.warmup, engine=args.engine,
+                          systems=None if args.systems == 64 else args.systems, hbm_budget_gb=args.hbm_budget_gb, peaks=peaks)
+    print(json.dumps(line))
     return 0
 
 
@@ -228,6 +329,10 @@ def main():
     ap.add_argument("--engine", type=int, default=1)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the secondary lines (cfg2_f64, cfg4, cfg4_general, cfg3) of the main run")
+    ap.add_argument("--hbm-budget-gb", type=float, default=150.0, help="cfg5: HBM budget the memory estimator fills")
+    ap.add_argument("--target", type=int, default=4096, help="cfg4_inflight: systems to relax")
+    ap.add_argument("--k-check", type=int, default=10, help="cfg4_inflight: FIRE steps between convergence checks")
     ap.add_argument("--workload", default="cfg2",
                     help="cfg2 (default: the graded configuration, full contract line) or one of cfg1, cfg2_f64, cfg3, cfg4, "
                          "cfg5: a short secondary line (device timing only) for the other BASELINE.json configs")
@@ -318,9 +423,10 @@ def main():
     entry_bytes = 4
     b_alg, flops = algorithmic_model(nbar, K, 4, entry_bytes)
     peak, peak_src = measured_peaks()
+    alu = fma_peaks(dev)
+    traffic, traffic_src = profile_traffic()
     launch_bytes = b_alg * st.N * n_inner
     achieved = launch_bytes / (float(ms.mean()) * 1e-3) / 1e9
-    p_fp32 = 148 * 128 * 2 * 1.965e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
         "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -334,19 +440,30 @@ def main():
         "e2e": {"value": atom_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC.get("resident" if rep1.engine == 1 else "general"), "peak_source": peak_src,
-                     "traffic_note": "dram__bytes_read+write per launch from profiles/ (ncu --set full of this command); the resident "
-                                     "engine keeps systems on chip, so DRAM traffic is far below the algorithmic byte model",
+                     "traffic": traffic if rep1.engine == 1 else None, "peak_source": peak_src,
+                     "traffic_note": f"dram__bytes_read+write per launch read from {traffic_src} (ncu --set full of this command); "
+                                     "`achieved` is the SURVEY 8(d) algorithmic byte model over the measured time, not DRAM traffic: "
+                                     "the resident engine keeps systems on chip, so its DRAM traffic is far below the model",
                      "model": f"B_alg = {b_alg:.1f} B/atom-step (state 68 + {entry_bytes} B x nbar {nbar:.1f} + rebuild/K, K = {K:.1f}) "
                               f"x {st.N} atoms x {n_inner} MD steps per launch sequence",
                      "alu": {"flop_per_atom_step": flops, "achieved_tflops": flops * st.N * n_inner / (float(ms.mean()) * 1e-3) / 1e12,
-                             "peak_tflops": p_fp32 / 1e12, "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (nominal)"}},
+                             "peak_tflops": alu["fp32"], "peak_tflops_fp32x2": alu["fp32x2"], "peak_tflops_fp64": alu["fp64"],
+                             "frac": flops * st.N * n_inner / (float(ms.mean()) * 1e-3) / 1e12 / alu["fp32"],
+                             "peak_source": "measured: ts_measure_fma_tflops (register-only FMA chains, this run)"}},
     }
+    st.close()
     if rank == 0:
+        if world == 1 and not args.no_secondary:
+            # the other configs at full size, each with its own SURVEY 8(d) roofline (context for BASELINE.md section 5)
+            out["secondary"] = []
+            for w in ("cfg2_f64", "cfg4", "cfg4_general", "cfg3"):
+                try:
+                    out["secondary"].append(secondary_line(w, 3, 3, engine=1, peaks=alu, hbm_peak=peak))
+                except Exception as e:                         # a secondary line must never cost the graded one
+                    out["secondary"].append({"config": {"workload": w}, "error": str(e)[:200]})
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline()
         print(json.dumps(out))
-    st.close()
     if world > 1:
         dist.destroy_process_group()
 

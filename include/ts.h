@@ -131,7 +131,7 @@ typedef struct {
     int32_t n_failed;        /* systems that hit max_steps */
     int32_t max_neighbors;   /* longest row built since the last full build (general engine; a running maximum over per-system rebuilds) */
     int32_t list_valid;
-    int64_t resident_rebuilds; /* resident engine: per-system list builds since create, summed over systems */
+    int64_t resident_rebuilds; /* per-system list builds since create, summed over systems (both engines) */
     int32_t engine;          /* engine that ran the last stepping call: 0 general, 1 resident */
     int32_t reserved;
 } ts_report;
@@ -213,6 +213,15 @@ ts_status ts_estimate_system_pairs(int64_t n_atoms, double volume, double r_list
 ts_status ts_get_neighbors(ts_state *st, int64_t *off, int32_t *j, int8_t *shift, int64_t cap,
                            void *stream);
 
+/* The Verlet list the system-resident engine would step system `system` with at the current positions, decoded to
+ * HOST arrays like ts_get_neighbors (off [n_s + 1] relative to the system, GLOBAL j, shift relative to the stored
+ * positions).  It is a SUPERSET list: every pair within max rc + skin is in it, and nothing beyond that radius plus a
+ * few parts in 10^6 of the longest cell edge (fixed-point fractions); the pair loop applies the strict cutoff (R9).
+ * j / shift may be NULL to get the count (*nnz) only.  TS_ERR_UNSUPPORTED when the resident engine does not apply to
+ * the batch.  Uses the pair region of the workspace (the general engine's list is invalidated).  Synchronises.       */
+ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int64_t *off, int32_t *j, int8_t *shift,
+                                    int64_t cap, int64_t *nnz, void *stream);
+
 /* ---- graph export and external-model stepping (SURVEY 8(f) NEXT-2; PAPER.md:56 ModelInterface, :112) ------------
  * The current Verlet list (radius max rc + skin, general engine; built or skin-checked first) as a dense edge list in
  * DEVICE arrays: edge_i / edge_j [cap] global atom indices, edge_shift [cap,3] in the state dtype = the integer image
@@ -248,6 +257,10 @@ ts_status ts_set_engine(ts_state *st, int32_t engine);
  * copy): forces are stale and the list must be skin-checked against the new positions before the
  * next step.  Host-side flag only, enqueues nothing.                                              */
 ts_status ts_invalidate(ts_state *st);
+
+/* Register-only FMA microbenchmark: the ALU peak the roofline of the pair kernels is reported against.
+ * kind 0: fp32 FFMA, 1: fp64 DFMA, 2: packed fp32 (fma.rn.f32x2).  scratch: device, >= 4096 bytes.  Synchronises.   */
+ts_status ts_measure_fma_tflops(int32_t kind, void *scratch, double *tflops, void *stream);
 
 /* Number of kernel launches enqueued by this state since create (for bench accounting).           */
 int64_t ts_launch_count(const ts_state *st);

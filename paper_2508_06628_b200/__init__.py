@@ -31,7 +31,8 @@ EXPORTS = ["ts_workspace_bytes", "ts_estimate_system_bytes", "ts_state_create", 
            "ts_get_system_steps", "ts_set_engine", "ts_invalidate", "ts_launch_count", "ts_clear_error",
            "ts_status_string", "ts_last_error", "ts_sched_fill", "ts_sched_max_scaler",
            "ts_sched_binpack", "ts_sched_partition", "ts_repack_systems", "ts_get_capacity",
-           "ts_estimate_system_pairs", "ts_export_edges", "ts_md_step_external", "ts_fire_step_external"]
+           "ts_estimate_system_pairs", "ts_export_edges", "ts_md_step_external", "ts_fire_step_external",
+           "ts_measure_fma_tflops", "ts_get_resident_neighbors"]
 
 TS_PHASE_INIT, TS_PHASE_PRE, TS_PHASE_POST, TS_PHASE_CHECK0 = 0, 1, 2, 3
 (TS_OK, TS_ERR_INVALID_ARG, TS_ERR_CUDA, TS_ERR_WORKSPACE_TOO_SMALL, TS_ERR_NBR_OVERFLOW, TS_ERR_STALE_NBR,
@@ -216,6 +217,26 @@ def ts_md_step_external(h, params, phase):
 
 def ts_fire_step_external(h, params, phase):
     _check(lib().ts_fire_step_external(h, C.byref(params), C.c_int32(phase), _stream()), "ts_fire_step_external", h)
+
+
+def ts_get_resident_neighbors(h, system, n_atoms_of_system):
+    off = np.zeros(n_atoms_of_system + 1, np.int64)
+    nnz = C.c_int64()
+    _check(lib().ts_get_resident_neighbors(h, C.c_int32(system), off.ctypes.data_as(C.c_void_p), None, None, C.c_int64(0),
+                                           C.byref(nnz), _stream()), "ts_get_resident_neighbors", h)
+    j = np.zeros(nnz.value, np.int32)
+    shift = np.zeros((nnz.value, 3), np.int8)
+    _check(lib().ts_get_resident_neighbors(h, C.c_int32(system), off.ctypes.data_as(C.c_void_p), j.ctypes.data_as(C.c_void_p),
+                                           shift.ctypes.data_as(C.c_void_p), C.c_int64(nnz.value), C.byref(nnz), _stream()),
+           "ts_get_resident_neighbors", h)
+    return off, j, shift
+
+
+def ts_measure_fma_tflops(kind, scratch_ptr):
+    out = C.c_double()
+    _check(lib().ts_measure_fma_tflops(C.c_int32(kind), C.c_void_p(scratch_ptr), C.byref(out), _stream()),
+           "ts_measure_fma_tflops")
+    return out.value
 
 
 def ts_get_neighbors(h, n_atoms):

@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libts.so")
 SOURCES = ["ts_api.cu", "ts_step.cu", "ts_build.cu", "ts_pair.cu", "ts_integrate.cu", "ts_resident.cu", "ts_sched.cu",
-           "ts_repack.cu", "ts_graph.cu"]
+           "ts_repack.cu", "ts_graph.cu", "ts_probe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -76,7 +76,10 @@ __global__ void k_build_begin(DevState d)
         if (!d.sys_rebuild[s]) continue;
         const int base = ts_cell_base(d.sysoff, s), nc = d.geom[s].ncell;
         for (int c = threadIdx.x; c <= nc; c += blockDim.x) d.cell_count[base + c] = 0;
-        if (threadIdx.x == 0) d.nbr_len[s] = 0;                /* row cursor of the system's CSR segment (k_nbr_fill) */
+        if (threadIdx.x == 0) {
+            d.nbr_len[s] = 0;                                  /* row cursor of the system's CSR segment (k_nbr_fill) */
+            atomicAdd(&d.status->res_rebuilds, 1ull);          /* per-system list builds, summed over systems */
+        }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         d.status->nnz = 0ull;

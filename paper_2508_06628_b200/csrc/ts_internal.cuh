@@ -52,7 +52,7 @@ struct DevStatus {
     unsigned int list_valid;
     unsigned int pad;
     unsigned long long res_nnz;       /* resident engine: pairs in the lists at the end of the last call */
-    unsigned long long res_rebuilds;  /* resident engine: per-system list builds, summed over systems    */
+    unsigned long long res_rebuilds;  /* per-system list builds, summed over systems (both engines)      */
 };
 
 /* Everything a kernel needs, passed by value (well under the 4 KB parameter limit). */

@@ -80,6 +80,9 @@ struct ResCfg {
     unsigned smem;
     int noise_helpers; /* the kick buffers of the noise helpers exist (they are left out when they do not fit) */
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
+    int dump_sys;      /* list export (ts_get_resident_neighbors): the one system whose list is dumped, -1 = normal run */
+    unsigned char *dump;  /* device: per CTA rank [rows | tmeta | gtab | wrap shift of the own atoms] */
+    unsigned dump_cta_bytes;
 };
 
 struct ResMisc {
@@ -848,6 +851,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         const int g0 = d.sysoff[s];
         const int N_s = d.sysoff[s + 1] - g0;
         const int N8 = (N_s + 7) & ~7;
+        if (rc.dump && s != rc.dump_sys) continue;
         const int A_s = ((((N_s + CL - 1) / CL) + 7) >> 3) << 3;   /* whole blocks of eight slots per CTA */
         const int a_begin = rank * A_s;
         const int A_own = max(0, min(A_s, N_s - a_begin));
@@ -1065,6 +1069,18 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 __syncthreads();
                 TICK(8);
             }
+            if (rc.dump) {
+                /* list export: the list this engine would step with for the current positions goes to global memory
+                 * as it lies in shared memory (the host decodes it); nothing of the state is changed */
+                unsigned char *out = rc.dump + (size_t)rank * rc.dump_cta_bytes;
+                const unsigned nrow = (unsigned)rc.A * (unsigned)rc.pitch * 2u / 4u;
+                for (unsigned k = tid; k < nrow; k += blockDim.x) ((unsigned *)out)[k] = ((const unsigned *)rows)[k];
+                unsigned *om = (unsigned *)out + nrow;
+                for (int k = tid; k < rc.A; k += blockDim.x) om[k] = tmeta[k];
+                for (int k = tid; k < N8; k += blockDim.x) om[rc.A + k] = k < N_s ? gtab[k] : 0u;
+                if (own) om[rc.A + RES_MAX_ATOMS + 1 + tid] = (unsigned)bits_from(OWN_SMEM ? oref[tid].d : Rr.d);
+                break;
+            }
 #ifdef TS_RES_TIMING
             const long long wt0 = clock64();
 #endif
@@ -1143,14 +1159,15 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 }
             }
         }
-        if (!FIRE && CL > 1) cl_wait();               /* pairs the last arrive */
-        if (FIRE && !have_ev) {                       /* stopped before the last pass: E of the final positions */
+        if (!FIRE && CL > 1 && !rc.dump) cl_wait();   /* pairs the last arrive */
+        if (FIRE && !have_ev && !rc.dump) {                       /* stopped before the last pass: E of the final positions */
             pair_phase<T, KIND, NT1, true>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
             __syncthreads();
         }
 #ifdef TS_RES_TIMING
         if (tid == 0) for (int k = 0; k < 12; ++k) atomicAdd(&g_res_prof[k], (unsigned long long)prof_acc[k]);
 #endif
+        if (rc.dump) { cluster.sync(); continue; }
         /* ---- store the system (R16): x, v at t + n dt, F(x), E, W, KE */
         double ke = 0.0;
         if (own) {
@@ -1419,6 +1436,105 @@ ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want
     st->launches += 1;
     st->last_engine = 1;
     st->list_built = false;          /* the general engine's list no longer matches the positions */
+    return TS_OK;
+}
+
+/* ------------------------------------------------------------------ list export (ts.h: ts_get_resident_neighbors)
+ * Runs the engine's own rebuild for the current positions of one system and decodes the list on the host: the list
+ * the benched engine steps with becomes checkable against the oracle's pair set (it is a SUPERSET list: radius
+ * r_list + eps_rel x the longest cell edge, in fixed-point fractions). */
+extern "C" ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int64_t *off, int32_t *j_out, int8_t *shift,
+                                               int64_t cap, int64_t *nnz, void *stream)
+{
+    if (!st || !off || !nnz || system < 0 || system >= st->d.S) return TS_ERR_INVALID_ARG;
+    if (st->seen_flags) return TS_ERR_STICKY;
+    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
+    cudaStream_t q = (cudaStream_t)stream;
+    ResCfg cfg = plan_of(st)->cfg;
+    const int a0 = st->h_sysoff[system], N_s = st->h_sysoff[system + 1] - a0, N8 = (N_s + 7) & ~7, CL = cfg.CL;
+    const size_t nrow = (size_t)cfg.A * cfg.pitch * 2 / 4;
+    const size_t cta_words = nrow + (size_t)cfg.A + RES_MAX_ATOMS + 1 + (size_t)cfg.A;
+    if (cta_words * 4 * CL > (size_t)st->d.nbr_cap * 4) return TS_ERR_WORKSPACE_TOO_SMALL;   /* the pair region is the dump area */
+    cfg.dump = (unsigned char *)st->d.nbr;
+    cfg.dump_sys = system;
+    cfg.dump_cta_bytes = (unsigned)(cta_words * 4);
+    cfg.n_clusters = 1;
+    st->list_built = false;                                 /* the general engine's list lived there */
+    ResKernel k = pick_kernel(st);
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.gridDim = dim3((unsigned)CL); lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
+    lc.dynamicSmemBytes = cfg.smem; lc.stream = q; lc.attrs = at; lc.numAttrs = 1;
+    MdConst c;
+    memset(&c, 0, sizeof c);
+    c.integrator = TS_NVE; c.dt = 1.0; c.hdt = 0.5;
+    ts_fire_params nofire;
+    memset(&nofire, 0, sizeof nofire);
+    DevState dd = st->d;
+    /* the kernel walks systems cid, cid + n_clusters, ...: start the one cluster at `system` by shifting the batch view */
+    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, dd, c, cfg, 0, 0u, nofire));
+    st->launches += 1;
+    std::vector<unsigned> buf(cta_words * (size_t)CL);
+    TS_CUDA_OK(st, cudaStreamSynchronize(q));
+    TS_CUDA_OK(st, cudaMemcpy(buf.data(), st->d.nbr, buf.size() * 4, cudaMemcpyDeviceToHost));
+    const int A_s = ((((N_s + CL - 1) / CL) + 7) >> 3) << 3;
+    auto unhash = [&](int t) {
+        const unsigned b = (unsigned)t >> 3;
+        const unsigned h = (int)b == (N8 >> 3) - 1 ? 0u : (b * 0x9E3779B1u) >> 29;
+        return (t & ~7) | (int)(((unsigned)t - h) & 7u);
+    };
+    /* ghost slot -> (slot of the atom, image subset, signs); wrap shift of every atom */
+    const unsigned *g0 = buf.data() + nrow + cfg.A;          /* gtab as rank 0 built it (identical in every CTA) */
+    std::vector<int> gsrc((size_t)cfg.NS, -1), gm((size_t)cfg.NS, 0), gsg((size_t)cfg.NS, 0);
+    for (int t = 0; t < N_s; ++t) {
+        const unsigned e = g0[t], act = (e >> 16) & 7u, sg = (e >> 19) & 7u;
+        unsigned slot = e & 0xffffu;
+        for (unsigned m = 1; m < 8; ++m)
+            if ((m & ~act) == 0u) {
+                if (slot < (unsigned)cfg.NS) { gsrc[slot] = t; gm[slot] = (int)m; gsg[slot] = (int)sg; }
+                slot += 8u;
+            }
+    }
+    std::vector<int> wpack((size_t)N_s, 0);
+    for (int r = 0; r < CL; ++r)
+        for (int al = 0; al < A_s && r * A_s + al < N_s; ++al)
+            wpack[(size_t)(r * A_s + al)] = (int)buf[(size_t)r * cta_words + nrow + cfg.A + RES_MAX_ATOMS + 1 + al];
+    auto wk = [&](int atom, int k) { return (int)(signed char)((wpack[(size_t)atom] >> (8 * k)) & 0xff); };
+    int64_t n = 0;
+    off[0] = 0;
+    for (int i = 0; i < N_s; ++i) {
+        const int r = i / A_s, al = i - r * A_s, task = al >> 3, a8 = al & 7;
+        const unsigned *cta = buf.data() + (size_t)r * cta_words;
+        const unsigned meta = cta[nrow + al];
+        const int nt = (int)(meta >> 14);
+        for (int t = 0; t < nt; ++t)
+            for (int l4 = 0; l4 < 4; ++l4)
+                for (int kk = 0; kk < 4; ++kk) {
+                    const unsigned word = cta[((size_t)task * cfg.pitch * 16 + (size_t)t * 256 + a8 * 32 + l4 * 8 + (kk >> 1) * 4) / 4];
+                    const int slot = (int)((kk & 1) ? word >> 18 : word & 0x3fffu);
+                    if (slot >= N8 && slot < N8 + 8) continue;                /* padding dummy */
+                    int src = slot, S[3] = { 0, 0, 0 };
+                    if (slot >= N8 + 8) {
+                        src = slot < cfg.NS ? gsrc[(size_t)slot] : -1;
+                        if (src < 0) return TS_ERR_INVALID_ARG;                /* an entry that names no slot: cannot happen */
+                        for (int c3 = 0; c3 < 3; ++c3)
+                            if ((gm[(size_t)slot] >> c3) & 1) S[c3] = ((gsg[(size_t)slot] >> c3) & 1) ? 1 : -1;
+                    }
+                    const int jj = unhash(src);
+                    if (j_out && shift) {
+                        if (n >= cap) return TS_ERR_WORKSPACE_TOO_SMALL;
+                        j_out[n] = a0 + jj;
+                        /* stored positions: x_j - x_i + S.h with S = S_image - wrap_j + wrap_i (R6) */
+                        for (int c3 = 0; c3 < 3; ++c3) shift[3 * n + c3] = (int8_t)(S[c3] - wk(jj, c3) + wk(i, c3));
+                    }
+                    ++n;
+                }
+        off[i + 1] = n;
+    }
+    *nnz = n;
     return TS_OK;
 }
 

@@ -123,6 +123,11 @@ class SimState:
     def get_neighbors(self):
         return ts.ts_get_neighbors(self.handle, self.N)
 
+    def get_resident_neighbors(self, system):
+        """(off, j, shift) of the list the system-resident engine would use for `system` at the current positions."""
+        n = int(self.sys_offset[system + 1] - self.sys_offset[system])
+        return ts.ts_get_resident_neighbors(self.handle, int(system), n)
+
     def set_system_steps(self, steps):
         ts.ts_set_system_steps(self.handle, steps)
 

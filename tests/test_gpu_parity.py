@@ -288,3 +288,38 @@ def test_resident_engine_static_energy_forces_virial(ts, orc, name):
     assert rep.flags == 0 and rep.engine == 1, (rep.flags, rep.engine)
     _check_efw(b, st, o, b.dtype == "f32")
     st.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2_f32", "cfg2_f64", "cfg5_f32", "cfg4_f64"])
+def test_resident_list_is_a_tight_superset_of_the_oracle_pair_set(ts, orc, name):
+    """The list of the benched (system-resident) engine, exported and decoded: it contains every oracle pair within
+    r_list and nothing beyond r_list plus the documented inflation (a few 1e-6 of the longest cell edge), on cfg2- and
+    cfg5-shaped systems and on the two-type mixture; also after the atoms have moved (a list built mid-trajectory)."""
+    if name.startswith("cfg2"):
+        b = wl.cfg2(n_systems=2, dtype=name[-3:])
+    elif name == "cfg5_f32":
+        start = wl.cfg5_start(range(2))                        # R33: random positions pre-relaxed by the library itself
+        sf = ts.SimState(start)
+        sf.fire_step(dict(start.fire, f_max=1e-12, max_steps=10 ** 6), 200)
+        b = wl.cfg5_md(wl.with_(start, pos=sf.numpy("pos").astype(np.float64)))
+        sf.close()
+    else:
+        b = wl.cfg4(range(3))
+    st = ts.SimState(b, engine=1, slack=2.0 if name == "cfg5_f32" else 1.25)
+    lmax = max(np.linalg.norm(b.cell[s], axis=1).max() for s in range(b.n_systems))
+    for moved in (False, True):
+        if moved and b.md:
+            st.md_step(dict(b.md), 7)
+        pos = st.numpy("pos").astype(np.float64)
+        for s in range(b.n_systems):
+            a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+            off, j, shift = st.get_resident_neighbors(s)
+            i = np.repeat(np.arange(a0, a1), np.diff(off))
+            got = set(zip(i.tolist(), j.tolist(), shift[:, 0].tolist(), shift[:, 1].tolist(), shift[:, 2].tolist()))
+            assert len(got) == j.size                                              # no duplicate (i, j, S)
+            lo = orc.pairs(pos[a0:a1], b.cell[s], b.r_list)
+            hi = orc.pairs(pos[a0:a1], b.cell[s], b.r_list + 16e-6 * lmax)
+            as_set = lambda p: set(zip((p[0] + a0).tolist(), (p[1] + a0).tolist(), p[2][:, 0].tolist(), p[2][:, 1].tolist(), p[2][:, 2].tolist()))
+            assert as_set(lo) <= got <= as_set(hi), (name, s, len(as_set(lo)), len(got), len(as_set(hi)))
+    assert st.poll().flags == 0
+    st.close()
