@@ -263,7 +263,7 @@ def secondary_line(w, steps, warmup, engine=1, systems=None, hbm_budget_gb=150.0
             "higher_is_better": True, "data": "synthetic", "dtype": b.dtype, "secondary": True,
             "config": dict({"workload": w, "systems": b.n_systems, "atoms": b.n_atoms, "steps_per_call": inner,
                             "kind": "fire" if fire else b.md.get("integrator"), "us_per_inner_step": ms * 1e3 / inner,
-                            "engine": "resident" if rep.engine == 1 else "general", "flags": int(rep.flags),
+                            "engine": {0: "general", 1: "resident", 2: "resident + general (mixed dispatch)"}[int(rep.engine)], "flags": int(rep.flags),
                             "mean_neighbours": nbar, "steps_per_rebuild": K}, **extra),
             "clocks": clk,
             "roofline": {"bound": "hbm", "achieved": b_alg * value / 1e9, "peak": hbm_peak, "unit": "GB/s",

@@ -132,7 +132,7 @@ typedef struct {
     int32_t max_neighbors;   /* longest row built since the last full build (general engine; a running maximum over per-system rebuilds) */
     int32_t list_valid;
     int64_t resident_rebuilds; /* per-system list builds since create, summed over systems (both engines) */
-    int32_t engine;          /* engine that ran the last stepping call: 0 general, 1 resident */
+    int32_t engine;          /* engine that ran the last stepping call: 0 general, 1 resident, 2 both (mixed dispatch of a ragged batch) */
     int32_t reserved;
 } ts_report;
 
@@ -249,8 +249,10 @@ ts_status ts_set_system_steps(ts_state *st, const uint64_t *steps, void *stream)
 ts_status ts_get_system_steps(ts_state *st, uint64_t *steps, void *stream);
 
 /* Select the stepping engine: 0 = general multi-kernel path (any system size), 1 = system-resident
- * path (whole systems held in shared memory across steps) where the batch allows it, falling back
- * to 0 otherwise.  Default 1.  Results obey the same tolerances either way.                       */
+ * path (whole systems held in shared memory across steps) for every system it can hold (cell heights >= 2 r_list,
+ * <= 2048 atoms), in up to four size classes launched side by side; ts_md_step steps the other systems of a ragged
+ * batch with the general engine NEXT to it on a stream of its own (ts_fire_step: all systems or none).  Default 1.
+ * Results obey the same tolerances either way.                                                                     */
 ts_status ts_set_engine(ts_state *st, int32_t engine);
 
 /* Tell the library that the caller wrote desc.pos / desc.vel from outside (e.g. a host -> device

@@ -322,6 +322,7 @@ __global__ void k_nbr_finish(DevState d)
     if (!d.status->need_rebuild) return;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= d.S) return;
+    if (ts_skip(d, s)) return;
     const long long cap = d.nbr_base[s + 1] - d.nbr_base[s];
     long long len = d.nbr_len[s];
     if (d.sys_rebuild[s] && len > cap) {
@@ -345,7 +346,7 @@ void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, c
 
 __global__ void k_force_rebuild(DevState d)
 {
-    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < d.S; s += gridDim.x * blockDim.x) d.sys_rebuild[s] = 1;
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < d.S; s += gridDim.x * blockDim.x) d.sys_rebuild[s] = ts_skip(d, s) ? 0 : 1;
     if (blockIdx.x == 0 && threadIdx.x == 0) { d.status->need_rebuild = 1u; d.status->max_nbr = 0u; }
 }
 

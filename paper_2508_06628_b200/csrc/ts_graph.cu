@@ -64,6 +64,7 @@ __global__ void k_edge_fill(DevState d, const long long *edge_base, long long *e
 
 static void ensure_list_graph(ts_state *st, cudaStream_t q)
 {
+    ts_whole_batch_mode(st);
     if (!st->list_built) launch_build(st, true, q);
     else { launch_import(st, q); launch_build(st, false, q); }
 }

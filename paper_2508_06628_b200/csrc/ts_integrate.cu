@@ -33,8 +33,10 @@ __global__ void k_import(DevState d)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.N) return;
+    const int s = d.sysidx[i];
+    if (ts_skip(d, s)) return;
     const T *x = (const T *)d.pos + 3 * i;
-    publish_pos<T>(d, i, d.sysidx[i], x[0], x[1], x[2]);
+    publish_pos<T>(d, i, s, x[0], x[1], x[2]);
 }
 
 template <typename T>
@@ -43,6 +45,7 @@ __global__ void k_md_pre(DevState d, MdConst c)
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.N) return;
     int s = d.sysidx[i];
+    if (ts_skip(d, s)) return;
     T *x = (T *)d.pos + 3 * i, *v = (T *)d.vel + 3 * i;
     const T *f = (const T *)d.force + 3 * i;
     T im = (T)1 / (((const T *)d.mass)[i] * (T)d.mass_conv);
@@ -96,6 +99,9 @@ __global__ void k_md_post(DevState d, MdConst c, int want_ke)
     double ke = 0.0;
     if (valid) {
         s = d.sysidx[i];
+        valid = !ts_skip(d, s);
+    }
+    if (valid) {
         T *v = (T *)d.vel + 3 * i;
         const T *f = (const T *)d.force + 3 * i;
         T m = ((const T *)d.mass)[i];
@@ -118,6 +124,9 @@ __global__ void k_kinetic(DevState d)
     double ke = 0.0;
     if (valid) {
         s = d.sysidx[i];
+        valid = !ts_skip(d, s);
+    }
+    if (valid) {
         const T *v = (const T *)d.vel + 3 * i;
         double m = (double)((const T *)d.mass)[i];
         ke = 0.5 * m * d.mass_conv * ((double)v[0] * (double)v[0] + (double)v[1] * (double)v[1] + (double)v[2] * (double)v[2]);
@@ -341,6 +350,13 @@ __global__ void k_fire_count(DevState d, int *out /* [2] converged, failed */)
     if (st == TS_FIRE_FAILED) atomicAdd(&out[1], 1);
 }
 
+/* kinetic energies of the systems this engine steps (a memset would wipe those of the resident engine's systems) */
+__global__ void k_zero_kinetic(DevState d)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < d.S && !ts_skip(d, s)) d.kinetic[s] = 0.0;
+}
+
 /* ------------------------------------------------------------------ host launchers */
 #define ATOM_GRID(d) (unsigned)(((d).N + 255) / 256), 256
 #define SYS_GRID(d) (unsigned)(((d).S + 127) / 128), 128
@@ -355,12 +371,13 @@ void launch_import(ts_state *st, cudaStream_t q) { BY_DTYPE(st, k_import, ATOM_G
 void launch_md_pre(ts_state *st, const MdConst &c, cudaStream_t q) { BY_DTYPE(st, k_md_pre, ATOM_GRID(st->d), st->d, c); }
 void launch_md_post(ts_state *st, const MdConst &c, bool want_ke, cudaStream_t q)
 {
-    if (want_ke) cudaMemsetAsync(st->d.kinetic, 0, sizeof(double) * (size_t)st->d.S, q);
+    if (want_ke) { k_zero_kinetic<<<SYS_GRID(st->d), 0, q>>>(st->d); st->launches += 1; }
     BY_DTYPE(st, k_md_post, ATOM_GRID(st->d), st->d, c, want_ke ? 1 : 0);
 }
 void launch_kinetic(ts_state *st, cudaStream_t q)
 {
-    cudaMemsetAsync(st->d.kinetic, 0, sizeof(double) * (size_t)st->d.S, q);
+    k_zero_kinetic<<<SYS_GRID(st->d), 0, q>>>(st->d);
+    st->launches += 1;
     BY_DTYPE(st, k_kinetic, ATOM_GRID(st->d), st->d);
 }
 void launch_fire_init(ts_state *st, const ts_fire_params &p, cudaStream_t q) { BY_DTYPE(st, k_fire_init, ATOM_GRID(st->d), st->d, p); }

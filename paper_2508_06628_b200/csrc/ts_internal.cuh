@@ -84,6 +84,9 @@ struct DevState {
     int *sys_rebuild;            /* [S] 1 = an atom of the system moved > skin/2: its list is rebuilt at the next build (R12) */
     unsigned long long *sys_step;/* [S] per-system step counter (R18)  */
     unsigned int *uid_own;       /* [S] persistent ids (copy or iota)  */
+    int *sys_engine;             /* [S] 1 = stepped by the system-resident engine (mixed dispatch of a ragged batch) */
+    int *res_list;               /* [S] the resident engine's systems, size class after size class */
+    int mixed;                   /* 1: this launch sequence of the general engine skips the systems with sys_engine = 1 */
     /* workspace: per atom */
     void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
     double4 *spos;               /* [N] sorted wrapped coords + local idx */
@@ -109,6 +112,7 @@ struct ts_state {
     int S_cap;
     bool list_built;             /* a build has been enqueued and no swap since */
     bool forces_current;
+    bool list_mixed;             /* the general engine's list covers only the systems the resident engine does not step */
     int engine;
     int last_engine;             /* engine that ran the last stepping call */
     void *res_plan;              /* resident engine launch plan (ts_resident.cu) */
@@ -122,7 +126,7 @@ struct ts_state {
 struct TsLayout {
     size_t total;
     size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
-        sys_active, sys_rebuild, sys_step, uid_own, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, pos4, spos, xref, cell_count, cell_start, atom_cell,
         atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
 };
 TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);
@@ -140,6 +144,8 @@ void ts_set_error(ts_state *st, const char *fmt, ...);
 
 /* ts_api.cu */
 long long ts_system_pair_capacity(long long n, double vol, double r_list, double slack);
+/* ts_step.cu: the general engine is about to work on the WHOLE batch: a list built for a mixed dispatch is stale */
+void ts_whole_batch_mode(ts_state *st);
 /* ts_build.cu */
 void launch_geometry(ts_state *st, int s_first, int s_count, const int *slots, cudaStream_t q);
 void launch_build(ts_state *st, bool force, cudaStream_t q);
@@ -159,6 +165,9 @@ void launch_fire_count(ts_state *st, cudaStream_t q);
 void launch_swap(ts_state *st, int n, const ts_state_desc *fresh, cudaStream_t q);
 /* ts_resident.cu */
 bool resident_supported(ts_state *st);
+int resident_general_count(ts_state *st);
+cudaStream_t resident_fork_general(ts_state *st, cudaStream_t q);
+void resident_join_general(ts_state *st, cudaStream_t q);
 void resident_invalidate(ts_state *st);
 void resident_free(ts_state *st);
 ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q);
@@ -170,6 +179,8 @@ template <> struct Vec4<float> { typedef float4 type; };
 template <> struct Vec4<double> { typedef double4 type; };
 
 __device__ __forceinline__ int ts_cell_base(const int *sysoff, int s) { return sysoff[s] + s; }
+/* mixed dispatch: the system belongs to the resident engine, the general engine's kernels leave it alone */
+__device__ __forceinline__ bool ts_skip(const DevState &d, int s) { return d.mixed && d.sys_engine[s]; }
 
 __device__ __forceinline__ unsigned int ts_pack_nbr(int j, int s0, int s1, int s2)
 {

@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256, 3) k_pair(DevState d, int masked)
     int sub = threadIdx.x & (LPA - 1);
     bool valid = i < d.N;
     int s = valid ? d.sysidx[i] : -1;
-    bool act = valid && !(masked && !d.sys_active[s]) && d.nbr_len[s] >= 0;
+    bool act = valid && !(masked && !d.sys_active[s]) && !ts_skip(d, s) && d.nbr_len[s] >= 0;
     const V4 *pos4 = (const V4 *)d.pos4;
     const PotEntry<T> *tab = (const PotEntry<T> *)d.pot;
     int nt = d.n_types;
@@ -139,6 +139,7 @@ __global__ void k_zero_ev(DevState d, int masked, unsigned want)
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= d.S) return;
     if (masked && !d.sys_active[s]) return;
+    if (ts_skip(d, s)) return;
     if (d.nbr_len[s] < 0) return;
     d.energy[s] = 0.0;
     if ((want & TS_WANT_VIRIAL) && d.virial)

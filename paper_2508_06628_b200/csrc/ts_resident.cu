@@ -65,7 +65,7 @@ namespace cg = cooperative_groups;
 
 #define RES_MAX_THREADS 896         /* fp32; the fp64 kernels need twice the registers: 512 */
 #define RES_MAX_THREADS_F64 512
-#define RES_MAX_ATOMS 2047          /* builder hit masks cover 8 x 256 candidates */
+#define RES_MAX_ATOMS 2048          /* builder hit masks cover 8 x 256 candidates */
 #define RES_MAX_SLOTS 16376         /* list entries are 16-bit slot numbers; shared memory is the real limit */
 #define RES_SMEM_LIMIT (227 * 1024)
 
@@ -80,6 +80,8 @@ struct ResCfg {
     unsigned smem;
     int noise_helpers; /* the kick buffers of the noise helpers exist (they are left out when they do not fit) */
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
+    const int *syslist; /* device: the systems this launch steps (one size class of the batch); NULL = 0 .. n_list - 1 */
+    int n_list;
     int dump_sys;      /* list export (ts_get_resident_neighbors): the one system whose list is dumped, -1 = normal run */
     unsigned char *dump;  /* device: per CTA rank [rows | tmeta | gtab | wrap shift of the own atoms] */
     unsigned dump_cta_bytes;
@@ -800,7 +802,7 @@ __device__ __forceinline__ void fire_reduce(cg::cluster_group &cluster, int CL, 
 }
 
 /* ------------------------------------------------------------------ the kernel */
-template <typename T, int KIND, bool NT1, bool FIRE>
+template <typename T, int KIND, bool NT1, bool FIRE, bool DUMP = false>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THREADS_F64, 1) k_resident_md(DevState d, MdConst c, ResCfg rc, int n_steps, unsigned want, ts_fire_params fp)
 {
     unsigned char *const smem = ts_smem;
@@ -847,11 +849,12 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
 
-    for (int s = cid; s < d.S; s += rc.n_clusters) {
+    for (int ks = cid; ks < rc.n_list; ks += rc.n_clusters) {
+        const int s = rc.syslist ? rc.syslist[ks] : ks;
         const int g0 = d.sysoff[s];
         const int N_s = d.sysoff[s + 1] - g0;
         const int N8 = (N_s + 7) & ~7;
-        if (rc.dump && s != rc.dump_sys) continue;
+        if (DUMP && s != rc.dump_sys) continue;
         const int A_s = ((((N_s + CL - 1) / CL) + 7) >> 3) << 3;   /* whole blocks of eight slots per CTA */
         const int a_begin = rank * A_s;
         const int A_own = max(0, min(A_s, N_s - a_begin));
@@ -1069,7 +1072,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 __syncthreads();
                 TICK(8);
             }
-            if (rc.dump) {
+            if (DUMP) {
                 /* list export: the list this engine would step with for the current positions goes to global memory
                  * as it lies in shared memory (the host decodes it); nothing of the state is changed */
                 unsigned char *out = rc.dump + (size_t)rank * rc.dump_cta_bytes;
@@ -1159,15 +1162,15 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 }
             }
         }
-        if (!FIRE && CL > 1 && !rc.dump) cl_wait();   /* pairs the last arrive */
-        if (FIRE && !have_ev && !rc.dump) {                       /* stopped before the last pass: E of the final positions */
+        if (!FIRE && CL > 1 && !DUMP) cl_wait();   /* pairs the last arrive */
+        if (FIRE && !have_ev && !DUMP) {                       /* stopped before the last pass: E of the final positions */
             pair_phase<T, KIND, NT1, true>(rc, pos_sa, rows_sa, tmeta, tab, fs, A_own, NT, red);
             __syncthreads();
         }
 #ifdef TS_RES_TIMING
         if (tid == 0) for (int k = 0; k < 12; ++k) atomicAdd(&g_res_prof[k], (unsigned long long)prof_acc[k]);
 #endif
-        if (rc.dump) { cluster.sync(); continue; }
+        if (DUMP) { cluster.sync(); continue; }
         /* ---- store the system (R16): x, v at t + n dt, F(x), E, W, KE */
         double ke = 0.0;
         if (own) {
@@ -1209,10 +1212,24 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
 }
 
 /* ------------------------------------------------------------------ host side */
-struct ResPlan {
-    bool checked, ok;
+/* A ragged batch is stepped in up to four SIZE CLASSES (<= 256, <= 512, <= 1024, <= 2048 atoms), each with its own
+ * launch shape and its own launch, side by side on their own streams; systems the engine cannot hold (a cell height
+ * below 2 r_list, too many atoms, no shape that fits shared memory) stay with the general engine, which then runs
+ * next to the resident launches on a stream of its own (ts_step.cu). */
+#define RES_MAX_CLASSES 4
+struct ResClass {
     ResCfg cfg;
     int fire_clusters;     /* clusters in flight of the FIRE kernel (0 = not asked yet) */
+    int n, list_off;       /* systems of the class: d.res_list[list_off .. list_off + n) */
+};
+struct ResPlan {
+    bool checked;
+    int n_classes, n_general;
+    ResClass cls[RES_MAX_CLASSES];
+    int *cls_of_sys;       /* host [S]: class of every system, -1 = general engine */
+    bool streams;
+    cudaStream_t aux[RES_MAX_CLASSES + 1];
+    cudaEvent_t ev_start, ev_done[RES_MAX_CLASSES + 1];
 };
 static ResPlan *plan_of(ts_state *st) { return (ResPlan *)st->res_plan; }
 
@@ -1279,47 +1296,41 @@ static bool res_layout(ResCfg &c, int CL, int nmax, int need_row, int need_slots
     return res_layout_n(c, CL, nmax, need_row, need_slots, dtype, n_types, thread_div, 0);
 }
 
-/* Decides once per batch geometry whether the resident engine applies and how it is launched. */
-bool resident_supported(ts_state *st)
+/* what one system asks of a launch shape */
+struct SysNeed { bool eligible; double nbar, slots; };
+
+static SysNeed system_need(const DevState &d, const SysGeom &g, int n, float eps_rel)
 {
-    if (!st->res_plan) st->res_plan = calloc(1, sizeof(ResPlan));
-    ResPlan *p = plan_of(st);
-    if (p->checked) return p->ok;
-    p->checked = true; p->ok = false; p->fire_clusters = 0;
-    const DevState &d = st->d;
-    int S = d.S;
-    std::vector<SysGeom> geo((size_t)S);
-    if (cudaMemcpy(geo.data(), d.geom, sizeof(SysGeom) * (size_t)S, cudaMemcpyDeviceToHost) != cudaSuccess) return false;
-    const float eps_rel = 4e-6f;
-    int nmax = 0;
-    double need = 0.0, need_slots = 0.0;
-    for (int s = 0; s < S; ++s) {
-        int n = st->h_sysoff[s + 1] - st->h_sysoff[s];
-        nmax = n > nmax ? n : nmax;
-        const SysGeom &g = geo[(size_t)s];
-        double lmax = 0.0;
-        for (int a = 0; a < 3; ++a)
-            lmax = fmax(lmax, sqrt(g.h[3 * a] * g.h[3 * a] + g.h[3 * a + 1] * g.h[3 * a + 1] + g.h[3 * a + 2] * g.h[3 * a + 2]));
-        double rb = d.r_list + 4.0 * eps_rel * lmax;
-        double images = 1.0, images2 = 1.0;                       /* E[c + 1], E[(c + 1)^2] of the image count c of an atom */
-        for (int k = 0; k < 3; ++k) {
-            if (!(g.hperp[k] >= 2.0 * rb)) return false;          /* more than one image within r_list possible */
-            const double pk = fmin(1.0, 2.0 * rb / g.hperp[k]);   /* an atom is within rb of a face of axis k */
-            images *= 1.0 + pk;
-            images2 *= 1.0 + 3.0 * pk;
-        }
-        double nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
-        need = fmax(need, nbar);
-        /* atoms + dummies + ghosts.  The ghosts of a bank group occupy one of eight interleaved slot sequences, so the
-         * array needs 8 x the fullest group: mean + z sigma of a sum of n / 8 independent image counts, + 8 per group.
-         * z = 6: 4 sigma overflowed a few of the 10^6 group fills of a 10^4-system liquid batch; a lattice written cell
-         * by cell deviates systematically by ~2.5 sigma (measured on configs[1]).  An overflow is always detected and
-         * flagged (TS_FLAG_NBR_OVERFLOW), never silent. */
-        const double mean_c = images - 1.0, var_c = fmax(0.0, (images2 - 2.0 * images + 1.0) - mean_c * mean_c);
-        const double sd_g = sqrt(var_c * n / 8.0);
-        need_slots = fmax(need_slots, ((n + 7) & ~7) + 8 + 8.0 * ceil(mean_c * n / 8.0 + 6.0 * sd_g + 8.0));
+    SysNeed r = { false, 0.0, 0.0 };
+    if (n > RES_MAX_ATOMS) return r;
+    double lmax = 0.0;
+    for (int a = 0; a < 3; ++a)
+        lmax = fmax(lmax, sqrt(g.h[3 * a] * g.h[3 * a] + g.h[3 * a + 1] * g.h[3 * a + 1] + g.h[3 * a + 2] * g.h[3 * a + 2]));
+    const double rb = d.r_list + 4.0 * eps_rel * lmax;
+    double images = 1.0, images2 = 1.0;                       /* E[c + 1], E[(c + 1)^2] of the image count c of an atom */
+    for (int k = 0; k < 3; ++k) {
+        if (!(g.hperp[k] >= 2.0 * rb)) return r;              /* more than one image within r_list possible */
+        const double pk = fmin(1.0, 2.0 * rb / g.hperp[k]);   /* an atom is within rb of a face of axis k */
+        images *= 1.0 + pk;
+        images2 *= 1.0 + 3.0 * pk;
     }
-    if (nmax > RES_MAX_ATOMS || d.n_types > TS_MAX_TYPES) return false;
+    r.eligible = true;
+    r.nbar = (double)n / g.vol * (4.0 / 3.0) * M_PI * rb * rb * rb;
+    /* atoms + dummies + ghosts.  The ghosts of a bank group occupy one of eight interleaved slot sequences, so the
+     * array needs 8 x the fullest group: mean + z sigma of a sum of n / 8 independent image counts, + 8 per group.
+     * z = 6: 4 sigma overflowed a few of the 10^6 group fills of a 10^4-system liquid batch; a lattice written cell
+     * by cell deviates systematically by ~2.5 sigma (measured on configs[1]).  An overflow is always detected and
+     * flagged (TS_FLAG_NBR_OVERFLOW), never silent. */
+    const double mean_c = images - 1.0, var_c = fmax(0.0, (images2 - 2.0 * images + 1.0) - mean_c * mean_c);
+    const double sd_g = sqrt(var_c * n / 8.0);
+    r.slots = ((n + 7) & ~7) + 8 + 8.0 * ceil(mean_c * n / 8.0 + 6.0 * sd_g + 8.0);
+    return r;
+}
+
+/* launch shape of one size class: S systems of at most nmax atoms, `need` neighbours per atom, need_slots position slots */
+static bool plan_class(ts_state *st, int S, int nmax, double need, double need_slots, float eps_rel, ResCfg &best_out)
+{
+    const DevState &d = st->d;
     double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
     int need_row = (int)ceil(need * slack);
     int dev = 0, nsm = 148;
@@ -1392,19 +1403,98 @@ bool resident_supported(ts_state *st)
     const bool ok0 = plan(need_slots, need_row, best, maxc, cost), okp = plan(need_slots, need_row_p, alt, maxc_p, cost_p);
     if (!ok0 && !okp) return false;
     if (okp && (!ok0 || cost_p <= 1.05 * cost)) { best = alt; maxc = maxc_p; }
-    if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)best.smem) != cudaSuccess) {
-        cudaGetLastError();
-        return false;
-    }
     best.eps_rel = eps_rel;
     if (getenv("TS_RES_VERBOSE"))
-        fprintf(stderr, "[ts resident] CL %d A %d pitch %d NS %d warps %d smem %u clusters %d of %d systems\n", best.CL, best.A,
-                best.pitch, best.NS, best.nwarps, best.smem, S < maxc ? S : maxc, S);
+        fprintf(stderr, "[ts resident] CL %d A %d pitch %d NS %d warps %d smem %u clusters %d of %d systems (<= %d atoms)\n", best.CL,
+                best.A, best.pitch, best.NS, best.nwarps, best.smem, S < maxc ? S : maxc, S, nmax);
     best.n_clusters = S < maxc ? S : maxc;
-    p->cfg = best;
-    p->ok = true;
+    best_out = best;
     return true;
 }
+
+/* Decides once per batch geometry which systems the resident engine steps, in which size classes and launch shapes.
+ * Reads the cell geometry back (synchronises). */
+static ResPlan *resident_plan(ts_state *st)
+{
+    if (!st->res_plan) st->res_plan = calloc(1, sizeof(ResPlan));
+    ResPlan *p = plan_of(st);
+    if (p->checked) return p;
+    p->checked = true; p->n_classes = 0; p->n_general = st->d.S;
+    const DevState &d = st->d;
+    const int S = d.S;
+    free(p->cls_of_sys);
+    p->cls_of_sys = (int *)malloc(sizeof(int) * (size_t)S);
+    for (int s = 0; s < S; ++s) p->cls_of_sys[s] = -1;
+    if (d.n_types > TS_MAX_TYPES) return p;
+    std::vector<SysGeom> geo((size_t)S);
+    if (cudaMemcpy(geo.data(), d.geom, sizeof(SysGeom) * (size_t)S, cudaMemcpyDeviceToHost) != cudaSuccess) return p;
+    const float eps_rel = 4e-6f;
+    const int bound[RES_MAX_CLASSES] = { 256, 512, 1024, RES_MAX_ATOMS };
+    std::vector<int> cls_of((size_t)S, -1), engine((size_t)S, 0), list;
+    std::vector<SysNeed> need((size_t)S);
+    int count[RES_MAX_CLASSES] = { 0, 0, 0, 0 };
+    for (int s = 0; s < S; ++s) {
+        const int n = st->h_sysoff[s + 1] - st->h_sysoff[s];
+        need[(size_t)s] = system_need(d, geo[(size_t)s], n, eps_rel);
+        if (!need[(size_t)s].eligible) continue;
+        int c = 0;
+        while (n > bound[c]) ++c;
+        cls_of[(size_t)s] = c;
+        count[c] += 1;
+    }
+    /* a class too small to fill even a few SMs joins the next larger one (its systems run in that shape) */
+    for (int c = 0; c + 1 < RES_MAX_CLASSES; ++c)
+        if (count[c] > 0 && count[c] < 8 && count[c + 1] > 0) {
+            for (int s = 0; s < S; ++s) if (cls_of[(size_t)s] == c) cls_of[(size_t)s] = c + 1;
+            count[c + 1] += count[c]; count[c] = 0;
+        }
+    unsigned max_smem = 0;
+    for (int c = 0; c < RES_MAX_CLASSES; ++c) {
+        if (!count[c]) continue;
+        int nmax = 0;
+        double nb = 0.0, slots = 0.0;
+        for (int s = 0; s < S; ++s)
+            if (cls_of[(size_t)s] == c) {
+                const int n = st->h_sysoff[s + 1] - st->h_sysoff[s];
+                nmax = n > nmax ? n : nmax;
+                nb = fmax(nb, need[(size_t)s].nbar); slots = fmax(slots, need[(size_t)s].slots);
+            }
+        ResClass &k = p->cls[p->n_classes];
+        memset(&k, 0, sizeof k);
+        if (!plan_class(st, count[c], nmax, nb, slots, eps_rel, k.cfg)) continue;       /* its systems stay with the general engine */
+        k.n = count[c]; k.list_off = (int)list.size();
+        for (int s = 0; s < S; ++s)
+            if (cls_of[(size_t)s] == c) { list.push_back(s); engine[(size_t)s] = 1; p->cls_of_sys[s] = p->n_classes; }
+        k.cfg.syslist = d.res_list + k.list_off;
+        k.cfg.n_list = k.n;
+        max_smem = k.cfg.smem > max_smem ? k.cfg.smem : max_smem;
+        p->n_classes += 1;
+    }
+    p->n_general = S - (int)list.size();
+    if (p->n_classes) {
+        if (cudaMemcpy(d.res_list, list.data(), sizeof(int) * list.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(d.sys_engine, engine.data(), sizeof(int) * (size_t)S, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaFuncSetAttribute((const void *)pick_kernel(st), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem) != cudaSuccess ||
+            cudaFuncSetAttribute((const void *)pick_kernel(st, true), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem) != cudaSuccess) {
+            cudaGetLastError();
+            p->n_classes = 0; p->n_general = S;
+            for (int s = 0; s < S; ++s) p->cls_of_sys[s] = -1;
+        }
+    }
+    if (getenv("TS_RES_VERBOSE"))
+        fprintf(stderr, "[ts resident] %d size class(es), %d of %d systems with the general engine\n", p->n_classes, p->n_general, S);
+    return p;
+}
+
+/* the resident engine steps the WHOLE batch (what ts_fire_step and the list export ask) */
+bool resident_supported(ts_state *st)
+{
+    ResPlan *p = resident_plan(st);
+    return p->n_classes > 0 && p->n_general == 0;
+}
+
+/* systems the general engine has to step next to the resident launches (0: none; S: the resident engine does not apply) */
+int resident_general_count(ts_state *st) { return resident_plan(st)->n_general; }
 
 void resident_invalidate(ts_state *st)
 {
@@ -1413,30 +1503,109 @@ void resident_invalidate(ts_state *st)
 
 void resident_free(ts_state *st)
 {
+    if (st->res_plan) {
+        ResPlan *p = plan_of(st);
+        if (p->streams) {
+            for (int k = 0; k <= RES_MAX_CLASSES; ++k) { cudaStreamDestroy(p->aux[k]); cudaEventDestroy(p->ev_done[k]); }
+            cudaEventDestroy(p->ev_start);
+        }
+        free(p->cls_of_sys);
+    }
     free(st->res_plan);
     st->res_plan = nullptr;
 }
 
+static bool plan_streams(ResPlan *p)
+{
+    if (p->streams) return true;
+    for (int k = 0; k <= RES_MAX_CLASSES; ++k)
+        if (cudaStreamCreateWithFlags(&p->aux[k], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_done[k], cudaEventDisableTiming) != cudaSuccess) return false;
+    if (cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) != cudaSuccess) return false;
+    p->streams = true;
+    return true;
+}
+
+/* The stream the general engine uses next to the resident launches of this call (fork from q), and the join. */
+cudaStream_t resident_fork_general(ts_state *st, cudaStream_t q)
+{
+    ResPlan *p = resident_plan(st);
+    if (!plan_streams(p)) return q;
+    cudaEventRecord(p->ev_start, q);
+    cudaStreamWaitEvent(p->aux[RES_MAX_CLASSES], p->ev_start, 0);
+    return p->aux[RES_MAX_CLASSES];
+}
+void resident_join_general(ts_state *st, cudaStream_t q)
+{
+    ResPlan *p = resident_plan(st);
+    if (!p->streams) return;
+    cudaEventRecord(p->ev_done[RES_MAX_CLASSES], p->aux[RES_MAX_CLASSES]);
+    cudaStreamWaitEvent(q, p->ev_done[RES_MAX_CLASSES], 0);
+}
+
+/* one launch per size class: the first on the caller's stream, the others on their own streams, joined at the end */
+static ts_status launch_classes(ts_state *st, bool fire, const MdConst &c, int n_steps, unsigned want, const ts_fire_params &fp,
+                                cudaStream_t q)
+{
+    ResPlan *p = resident_plan(st);
+    if (p->n_classes < 1) return TS_ERR_UNSUPPORTED;
+    if (p->n_classes > 1 && !plan_streams(p)) return TS_ERR_CUDA;
+    ResKernel k = pick_kernel(st, fire);
+    TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
+    if (p->n_classes > 1) TS_CUDA_OK(st, cudaEventRecord(p->ev_start, q));
+    for (int ci = 0; ci < p->n_classes; ++ci) {
+        ResClass &cl = p->cls[ci];
+        ResCfg cfg = cl.cfg;
+        cudaStream_t sq = ci == 0 ? q : p->aux[ci];
+        if (ci > 0) TS_CUDA_OK(st, cudaStreamWaitEvent(sq, p->ev_start, 0));
+        cudaLaunchConfig_t lc;
+        memset(&lc, 0, sizeof lc);
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)cfg.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
+        lc.dynamicSmemBytes = cfg.smem; lc.stream = sq; lc.attrs = at; lc.numAttrs = 1;
+        if (fire) {
+            if (cl.fire_clusters == 0) {               /* the FIRE variant has its own register count and occupancy */
+                lc.gridDim = dim3((unsigned)(cfg.CL * cl.n));
+                int maxc = 0;
+                if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
+                    cudaGetLastError();
+                    return TS_ERR_UNSUPPORTED;
+                }
+                cl.fire_clusters = cl.n < maxc ? cl.n : maxc;
+            }
+            cfg.n_clusters = cl.fire_clusters;
+        }
+        lc.gridDim = dim3((unsigned)(cfg.CL * cfg.n_clusters));
+        TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, want, fp));
+        st->launches += 1;
+        if (ci > 0) {
+            TS_CUDA_OK(st, cudaEventRecord(p->ev_done[ci], sq));
+            TS_CUDA_OK(st, cudaStreamWaitEvent(q, p->ev_done[ci], 0));
+        }
+    }
+    st->last_engine = p->n_general ? 2 : 1;
+    return TS_OK;
+}
+
+/* the resident share of an MD call: every size class; the general engine steps the other systems (ts_step.cu) */
 ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q)
 {
-    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
-    const ResCfg &cfg = plan_of(st)->cfg;
-    ResKernel k = pick_kernel(st);
-    TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof lc);
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)cfg.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    lc.gridDim = dim3((unsigned)(cfg.CL * cfg.n_clusters)); lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
-    lc.dynamicSmemBytes = cfg.smem; lc.stream = q; lc.attrs = at; lc.numAttrs = 1;
     ts_fire_params nofire;
     memset(&nofire, 0, sizeof nofire);
-    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, want, nofire));
-    st->launches += 1;
-    st->last_engine = 1;
-    st->list_built = false;          /* the general engine's list no longer matches the positions */
-    return TS_OK;
+    return launch_classes(st, false, c, n_steps, want, nofire, q);
+}
+
+/* FIRE relaxation inside the resident engine: the same kernel in FIRE mode (per-system dt, the four reductions and
+ * the state machine after every step, finished systems skipped bit-unchanged); whole batches only. */
+ts_status resident_fire(ts_state *st, const ts_fire_params &fp, int n_steps, cudaStream_t q)
+{
+    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
+    MdConst c;
+    memset(&c, 0, sizeof c);
+    c.integrator = TS_NVE;
+    return launch_classes(st, true, c, n_steps, (unsigned)TS_WANT_ENERGY, fp, q);
 }
 
 /* ------------------------------------------------------------------ list export (ts.h: ts_get_resident_neighbors)
@@ -1448,9 +1617,11 @@ extern "C" ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int
 {
     if (!st || !off || !nnz || system < 0 || system >= st->d.S) return TS_ERR_INVALID_ARG;
     if (st->seen_flags) return TS_ERR_STICKY;
-    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
+    ResPlan *pl = resident_plan(st);
+    if (pl->cls_of_sys[system] < 0) return TS_ERR_UNSUPPORTED;
     cudaStream_t q = (cudaStream_t)stream;
-    ResCfg cfg = plan_of(st)->cfg;
+    ResCfg cfg = pl->cls[pl->cls_of_sys[system]].cfg;
+    cfg.syslist = nullptr; cfg.n_list = st->d.S;
     const int a0 = st->h_sysoff[system], N_s = st->h_sysoff[system + 1] - a0, N8 = (N_s + 7) & ~7, CL = cfg.CL;
     const size_t nrow = (size_t)cfg.A * cfg.pitch * 2 / 4;
     const size_t cta_words = nrow + (size_t)cfg.A + RES_MAX_ATOMS + 1 + (size_t)cfg.A;
@@ -1460,7 +1631,12 @@ extern "C" ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int
     cfg.dump_cta_bytes = (unsigned)(cta_words * 4);
     cfg.n_clusters = 1;
     st->list_built = false;                                 /* the general engine's list lived there */
-    ResKernel k = pick_kernel(st);
+    ResKernel k = st->d.dtype == TS_F32 ? (ResKernel)k_resident_md<float, TS_LJ, false, false, true>
+                                        : (ResKernel)k_resident_md<double, TS_LJ, false, false, true>;   /* the build does not depend on the potential */
+    if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem) != cudaSuccess) {
+        cudaGetLastError();
+        return TS_ERR_CUDA;
+    }
     cudaLaunchConfig_t lc;
     memset(&lc, 0, sizeof lc);
     cudaLaunchAttribute at[1];
@@ -1556,45 +1732,4 @@ extern "C" int ts_debug_resident_profile(unsigned long long *out16)
     (void)out16;
     return 2;
 #endif
-}
-
-/* FIRE relaxation inside the resident engine: the same kernel in FIRE mode (per-system dt, the four reductions and
- * the state machine after every step, finished systems skipped bit-unchanged). */
-ts_status resident_fire(ts_state *st, const ts_fire_params &fp, int n_steps, cudaStream_t q)
-{
-    if (!resident_supported(st)) return TS_ERR_UNSUPPORTED;
-    ResPlan *p = plan_of(st);
-    ResCfg cfg = p->cfg;
-    ResKernel k = pick_kernel(st, true);
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof lc);
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)cfg.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    lc.blockDim = dim3((unsigned)(cfg.nwarps * 32));
-    lc.dynamicSmemBytes = cfg.smem; lc.stream = q; lc.attrs = at; lc.numAttrs = 1;
-    if (p->fire_clusters == 0) {                     /* the FIRE variant has its own register count and occupancy */
-        if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem) != cudaSuccess) {
-            cudaGetLastError();
-            return TS_ERR_UNSUPPORTED;
-        }
-        lc.gridDim = dim3((unsigned)(cfg.CL * st->d.S));
-        int maxc = 0;
-        if (cudaOccupancyMaxActiveClusters(&maxc, (const void *)k, &lc) != cudaSuccess || maxc < 1) {
-            cudaGetLastError();
-            return TS_ERR_UNSUPPORTED;
-        }
-        p->fire_clusters = st->d.S < maxc ? st->d.S : maxc;
-    }
-    cfg.n_clusters = p->fire_clusters;
-    lc.gridDim = dim3((unsigned)(cfg.CL * cfg.n_clusters));
-    TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
-    MdConst c;
-    memset(&c, 0, sizeof c);
-    c.integrator = TS_NVE;
-    TS_CUDA_OK(st, cudaLaunchKernelEx(&lc, k, st->d, c, cfg, n_steps, (unsigned)TS_WANT_ENERGY, fp));
-    st->launches += 1;
-    st->last_engine = 1;
-    st->list_built = false;          /* the general engine's list no longer matches the positions */
-    return TS_OK;
 }

@@ -28,6 +28,12 @@ static ts_status check_launch(ts_state *st)
         if ((st)->seen_flags) return TS_ERR_STICKY;     \
     } while (0)
 
+void ts_whole_batch_mode(ts_state *st)
+{
+    if (st->list_mixed) { st->list_built = false; st->forces_current = false; st->list_mixed = false; }
+    st->d.mixed = 0;
+}
+
 /* list for the current positions: forced build the first time, skin-checked afterwards */
 static void ensure_list(ts_state *st, cudaStream_t q)
 {
@@ -51,6 +57,7 @@ extern "C" ts_status ts_compute_forces(ts_state *st, uint32_t want, void *stream
     NEED_STATE(st);
     cudaStream_t q = (cudaStream_t)stream;
     st->last_engine = 0;
+    ts_whole_batch_mode(st);
     ensure_list(st, q);
     launch_pair(st, want & 3u, false, q);
     if (want & TS_WANT_ENERGY) launch_kinetic(st, q);
@@ -73,26 +80,48 @@ extern "C" ts_status ts_md_step(ts_state *st, const ts_md_params *p, int32_t n_s
     c.kT = st->d.kB * p->temperature;
     c.key0 = (unsigned)(p->seed & 0xffffffffull); c.key1 = (unsigned)(p->seed >> 32);
     want = (want & 3u) | TS_WANT_ENERGY;
-    if (st->engine == 1 && resident_supported(st)) {
+    /* Engine dispatch.  The resident engine steps every system it can hold, size class by size class; the general engine
+     * steps the others NEXT to it on a stream of its own (mixed dispatch of a ragged batch), or the whole batch when the
+     * resident engine is switched off or does not apply at all. */
+    const int n_general = st->engine == 1 ? resident_general_count(st) : st->d.S;
+    const bool use_resident = n_general < st->d.S, mixed = use_resident && n_general > 0;
+    if (use_resident) {
         ts_status rc = resident_md(st, c, n_steps, want, q);
-        if (rc != TS_ERR_UNSUPPORTED) {
-            if (rc == TS_OK) { st->steps_done += n_steps; st->forces_current = true; }
-            return rc;
+        if (rc != TS_OK) return rc;
+        if (!mixed) {
+            st->steps_done += n_steps;
+            st->forces_current = true;
+            st->list_built = false;          /* the general engine's list no longer matches the positions */
+            st->list_mixed = false;
+            return TS_OK;
         }
+    } else {
+        st->last_engine = 0;
     }
-    st->last_engine = 0;
+    cudaStream_t g = q;
+    if (mixed) {
+        if (!st->list_mixed) { st->list_built = false; st->forces_current = false; st->list_mixed = true; }
+        st->d.mixed = 1;
+        g = resident_fork_general(st, q);
+    } else {
+        ts_whole_batch_mode(st);
+    }
     if (!st->forces_current || !st->list_built || n_steps == 0) {   /* no list of its own yet (e.g. the resident engine ran before) */
-        ensure_list(st, q);
-        launch_pair(st, n_steps == 0 ? want : 0u, false, q);
-        if (n_steps == 0) launch_kinetic(st, q);
+        ensure_list(st, g);
+        launch_pair(st, n_steps == 0 ? want : 0u, false, g);
+        if (n_steps == 0) launch_kinetic(st, g);
         st->forces_current = true;
     }
     for (int n = 0; n < n_steps; ++n) {
         bool last = n == n_steps - 1;
-        launch_md_pre(st, c, q);
-        launch_build(st, false, q);
-        launch_pair(st, last ? want : 0u, false, q);
-        launch_md_post(st, c, last, q);
+        launch_md_pre(st, c, g);
+        launch_build(st, false, g);
+        launch_pair(st, last ? want : 0u, false, g);
+        launch_md_post(st, c, last, g);
+    }
+    if (mixed) {
+        resident_join_general(st, q);
+        st->d.mixed = 0;
     }
     st->steps_done += n_steps;
     return check_launch(st);
@@ -106,11 +135,12 @@ extern "C" ts_status ts_fire_step(ts_state *st, const ts_fire_params *p, int32_t
     if (st->engine == 1 && resident_supported(st)) {
         ts_status rc = resident_fire(st, *p, n_steps, q);
         if (rc != TS_ERR_UNSUPPORTED) {
-            if (rc == TS_OK) { st->steps_done += n_steps; st->forces_current = true; }
+            if (rc == TS_OK) { st->steps_done += n_steps; st->forces_current = true; st->list_built = false; st->list_mixed = false; }
             return rc;
         }
     }
     st->last_engine = 0;
+    ts_whole_batch_mode(st);
     launch_fire_init(st, *p, q);
     ensure_list(st, q);
     launch_pair(st, TS_WANT_ENERGY, true, q);
@@ -139,7 +169,7 @@ extern "C" ts_status ts_poll(ts_state *st, ts_report *out, void *stream)
     memset(out, 0, sizeof *out);
     out->flags = hs.flags;
     out->n_rebuilds = (int32_t)hs.n_rebuilds;
-    out->nnz = st->last_engine == 1 ? (int64_t)hs.res_nnz : (int64_t)hs.nnz;
+    out->nnz = st->last_engine == 1 ? (int64_t)hs.res_nnz : st->last_engine == 2 ? (int64_t)(hs.res_nnz + hs.nnz) : (int64_t)hs.nnz;
     out->resident_rebuilds = (int64_t)hs.res_rebuilds;
     out->engine = st->last_engine;
     out->nnz_capacity = st->d.nbr_cap;

@@ -323,3 +323,30 @@ def test_resident_list_is_a_tight_superset_of_the_oracle_pair_set(ts, orc, name)
             assert as_set(lo) <= got <= as_set(hi), (name, s, len(as_set(lo)), len(got), len(as_set(hi)))
     assert st.poll().flags == 0
     st.close()
+
+
+def test_mixed_engine_dispatch_of_a_ragged_batch(ts, orc):
+    """A ragged Morse batch (cfg3-shaped, 32..900 atoms): the systems whose cells are at least 2 r_list high run in the
+    system-resident engine, size class by size class, the small ones next to them in the general engine; every system
+    follows the oracle (fp64: positions to 1e-8 after 60 steps, E / KE / W), and a later whole-batch call still works."""
+    b = wl.cfg3(n_systems=24, dtype="f64", n_range=(32, 900))
+    o = orc.md_run(b, "nve", b.md["dt"], 60)
+    st = ts.SimState(b, engine=1)
+    st.md_step(dict(b.md), 25, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    st.md_step(dict(b.md), 35, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 2, (rep.flags, rep.engine)           # both engines stepped systems
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
+    assert np.allclose(st.numpy("energy"), o["E"], rtol=1e-10) and np.allclose(st.numpy("kinetic"), o["KE"], rtol=1e-10)
+    wscale = np.abs(o["W"]).reshape(b.n_systems, -1).max(1)
+    assert np.all(np.abs(st.numpy("virial") - o["W"]).reshape(b.n_systems, -1).max(1) <= 1e-9 * wscale)
+    assert np.array_equal(st.get_system_steps(), np.full(b.n_systems, 60, np.uint64))
+    st.compute_forces(ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)                     # whole batch through the general engine
+    assert st.poll().flags == 0
+    assert np.abs(st.numpy("force") - o["F"]).max() <= 1e-9
+    st.set_engine(0)
+    st.md_step(dict(b.md), 5)
+    o2 = orc.md_run(b, "nve", b.md["dt"], 65)
+    assert st.poll().engine == 0 and np.abs(st.numpy("pos") - o2["pos"]).max() <= 1e-8
+    st.close()
