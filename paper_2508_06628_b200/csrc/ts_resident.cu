@@ -390,6 +390,44 @@ __device__ __forceinline__ void lj_pair2(const float4 &pa, const float4 &pb, flo
     FZ = fma2(G, RZ, FZ);
 }
 
+/* the same for the fp32 Morse force loop: g = V'(r)/r = 2 D alpha (1 - e) e / r, e = exp(-alpha (r - r0)) as one ex2
+ * (NA = -alpha log2 e, AR = alpha r0 log2 e), 1 / r as one rsqrt */
+__device__ __forceinline__ void morse_pair2(const float4 &pa, const float4 &pb, float xix, float xiy, float xiz, float rc2,
+                                            f32x2 NA, f32x2 AR, f32x2 C0, f32x2 &FX, f32x2 &FY, f32x2 &FZ)
+{
+    const f32x2 RX = pk2(pa.x - xix, pb.x - xix), RY = pk2(pa.y - xiy, pb.y - xiy), RZ = pk2(pa.z - xiz, pb.z - xiz);
+    f32x2 R2 = mul2(RX, RX);
+    R2 = fma2(RY, RY, R2);
+    R2 = fma2(RZ, RZ, R2);
+    float r2a, r2b;
+    upk2(R2, r2a, r2b);
+    float ia, ib;
+    asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(ia) : "f"(r2a));      /* volatile: see lj_pair2 */
+    asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(ib) : "f"(r2b));
+    const float ma = r2a < rc2 ? 1.0f : 0.0f, mb = r2b < rc2 ? 1.0f : 0.0f;   /* strict (R9) */
+    const f32x2 IR = pk2(ia, ib);
+    const f32x2 X = fma2(mul2(R2, IR), NA, AR);        /* -alpha (r - r0) log2 e */
+    float xa, xb, ea, eb;
+    upk2(X, xa, xb);
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ea) : "f"(xa));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(eb) : "f"(xb));
+    const f32x2 E = pk2(ea, eb);
+    const f32x2 OM = fma2(E, pk2(-1.0f, -1.0f), pk2(1.0f, 1.0f));
+    const f32x2 G = mul2(mul2(mul2(C0, pk2(ma, mb)), OM), mul2(E, IR));
+    FX = fma2(G, RX, FX);
+    FY = fma2(G, RY, FY);
+    FZ = fma2(G, RZ, FZ);
+}
+
+/* one packed step of the fast loops: KIND selects the potential; A, B, C are its three packed constants */
+template <int KIND>
+__device__ __forceinline__ void fast_pair2(const float4 &pa, const float4 &pb, float xix, float xiy, float xiz, float rc2,
+                                           f32x2 A, f32x2 B, f32x2 C, f32x2 &FX, f32x2 &FY, f32x2 &FZ)
+{
+    if (KIND == TS_LJ) lj_pair2(pa, pb, xix, xiy, xiz, rc2, A, B, FX, FY, FZ);
+    else morse_pair2(pa, pb, xix, xiy, xiz, rc2, A, B, C, FX, FY, FZ);
+}
+
 /* ------------------------------------------------------------------ list layout
  * A TASK is eight consecutive own atoms, served by one warp: four lanes per atom (lane = 4 a + l4, a = atom of the
  * task, l4 = lane of the atom).  The list of an atom has eight COLUMNS, one per 16-byte bank group of the slot array
@@ -427,7 +465,7 @@ __device__ __forceinline__ T reduce3_4(T fx, T fy, T fz, int l4)
 }
 
 /* Forces of the CTA's own atoms from the shared-memory list; EV: energy and virial partials accumulate in fp64 (R31)
- * and end as warp partials in red.  FAST = fp32 Lennard-Jones, one type, forces only: two entries share packed f32x2
+ * and end as warp partials in red.  FAST = fp32 Lennard-Jones or Morse, one type, forces only: two entries share packed f32x2
  * operations, and the positions of the next two entries are gathered while the current two are computed. */
 template <typename T, int KIND, bool NT1, bool EV>
 __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, unsigned rows_sa, const unsigned *tmeta,
@@ -441,11 +479,15 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
     const int l4 = lane & 3, a8 = lane >> 2;
     const unsigned zt = (unsigned)rc.NS * 16u;
     const int ntasks = (A_own + 7) >> 3;
-    constexpr bool FAST = (sizeof(T) == 4) && KIND == TS_LJ && NT1 && !EV;
+    constexpr bool FAST = (sizeof(T) == 4) && (KIND == TS_LJ || KIND == TS_MORSE) && NT1 && !EV;
     const unsigned task_stride = (unsigned)rc.pitch * 16u;
     const unsigned lane_off = (unsigned)lane * 8u;
     const PotEntry<T> pe1 = tab[0];
-    const float rc2f = (float)pe1.rc2, m12 = -12.0f * (float)pe1.c0, p6 = 6.0f * (float)pe1.c1;
+    /* packed constants of the fast loops.  LJ: -12 c0, 6 c1.  Morse: -alpha log2 e, alpha r0 log2 e, 2 D alpha */
+    const float rc2f = (float)pe1.rc2;
+    const float ka = KIND == TS_LJ ? -12.0f * (float)pe1.c0 : -1.4426950408889634f * (float)pe1.p1;
+    const float kb = KIND == TS_LJ ? 6.0f * (float)pe1.c1 : 1.4426950408889634f * (float)pe1.p1 * (float)pe1.p2;
+    const float kc = (float)pe1.c0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
         const int al = task * 8 + a8;
         const unsigned meta = tmeta[al];
@@ -458,7 +500,7 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
         if (FAST) {
             const float4 xi4 = lds128(xa);
             const float xix = xi4.x, xiy = xi4.y, xiz = xi4.z;
-            const f32x2 C12 = pk2(m12, m12), C6 = pk2(p6, p6);
+            const f32x2 KA = pk2(ka, ka), KB = pk2(kb, kb), KC = pk2(kc, kc);
             f32x2 FX = pk2(0.f, 0.f), FY = FX, FZ = FX;
             if (nt > 0) {
                 uint2 w = lds64(ra);
@@ -466,13 +508,13 @@ __device__ __forceinline__ void pair_phase(const ResCfg &rc, unsigned pos_sa, un
                 for (int t = 1; t < nt; ++t) {
                     const float4 q0 = lds128(ent_even(w.y, pos_sa)), q1 = lds128(ent_odd(w.y, pos_sa));
                     w = lds64(ra + (unsigned)t * 256u);
-                    lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
+                    fast_pair2<KIND>(p0, p1, xix, xiy, xiz, rc2f, KA, KB, KC, FX, FY, FZ);
                     p0 = lds128(ent_even(w.x, pos_sa)); p1 = lds128(ent_odd(w.x, pos_sa));
-                    lj_pair2(q0, q1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
+                    fast_pair2<KIND>(q0, q1, xix, xiy, xiz, rc2f, KA, KB, KC, FX, FY, FZ);
                 }
                 const float4 q0 = lds128(ent_even(w.y, pos_sa)), q1 = lds128(ent_odd(w.y, pos_sa));
-                lj_pair2(p0, p1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
-                lj_pair2(q0, q1, xix, xiy, xiz, rc2f, C12, C6, FX, FY, FZ);
+                fast_pair2<KIND>(p0, p1, xix, xiy, xiz, rc2f, KA, KB, KC, FX, FY, FZ);
+                fast_pair2<KIND>(q0, q1, xix, xiy, xiz, rc2f, KA, KB, KC, FX, FY, FZ);
             }
             float a, b;
             upk2(FX, a, b); fx = (T)(a + b);
