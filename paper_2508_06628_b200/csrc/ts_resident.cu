@@ -1543,6 +1543,41 @@ void resident_invalidate(ts_state *st)
     if (st->res_plan) plan_of(st)->checked = false;
 }
 
+/* An equal-size swap brought new cells (HOST copy, [n, 9] in the state dtype) into `slots`: the plan stays when every
+ * new system still fits the launch shape of its slot's class (eligible, neighbours per row, position slots), so that an
+ * in-flight run does not re-plan (a device read and occupancy queries) at every swap. */
+void resident_after_swap(ts_state *st, const int32_t *slots, int n, const void *cells_host)
+{
+    if (!st->res_plan || !plan_of(st)->checked) return;
+    ResPlan *p = plan_of(st);
+    const DevState &d = st->d;
+    const double slack = st->nbr.slack >= 1.0 ? st->nbr.slack : 1.25;
+    for (int k = 0; k < n; ++k) {
+        const int s = slots[k], c = p->cls_of_sys ? p->cls_of_sys[s] : -1;
+        SysGeom g;
+        for (int e = 0; e < 9; ++e)
+            g.h[e] = d.dtype == TS_F32 ? (double)((const float *)cells_host)[9 * (size_t)k + e] : ((const double *)cells_host)[9 * (size_t)k + e];
+        const double *h = g.h;
+        const double c00 = h[4] * h[8] - h[5] * h[7], c01 = h[5] * h[6] - h[3] * h[8], c02 = h[3] * h[7] - h[4] * h[6];
+        const double det = h[0] * c00 + h[1] * c01 + h[2] * c02;
+        if (!(fabs(det) > 0.0)) { p->checked = false; return; }
+        const double id = 1.0 / det;
+        const double hinv[9] = { c00 * id, (h[2] * h[7] - h[1] * h[8]) * id, (h[1] * h[5] - h[2] * h[4]) * id,
+                                 c01 * id, (h[0] * h[8] - h[2] * h[6]) * id, (h[2] * h[3] - h[0] * h[5]) * id,
+                                 c02 * id, (h[1] * h[6] - h[0] * h[7]) * id, (h[0] * h[4] - h[1] * h[3]) * id };
+        g.vol = fabs(det);
+        for (int a = 0; a < 3; ++a) g.hperp[a] = 1.0 / sqrt(hinv[a] * hinv[a] + hinv[3 + a] * hinv[3 + a] + hinv[6 + a] * hinv[6 + a]);
+        const int natoms = st->h_sysoff[s + 1] - st->h_sysoff[s];
+        const SysNeed need = system_need(d, g, natoms, 4e-6f);
+        bool fits = c >= 0 ? need.eligible : !need.eligible;            /* a general-engine slot stays one only if it still has to */
+        if (c >= 0 && fits) {
+            const ResCfg &cfg = p->cls[c].cfg;
+            fits = (int)ceil(need.nbar * slack) <= cfg.pitch && need.slots <= (double)cfg.NS;
+        }
+        if (!fits) { p->checked = false; return; }
+    }
+}
+
 void resident_free(ts_state *st)
 {
     if (st->res_plan) {

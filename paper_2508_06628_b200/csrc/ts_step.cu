@@ -233,11 +233,17 @@ extern "C" ts_status ts_swap_systems(ts_state *st, const int32_t *slots, int32_t
     if (off != fresh->n_atoms) return TS_ERR_INVALID_ARG;
     TS_CUDA_OK(st, cudaMemcpyAsync(st->d.scratch, up.data(), sizeof(int) * up.size(), cudaMemcpyHostToDevice, q));
     launch_swap(st, n, fresh, q);
-    if (fresh->cell) { launch_geometry(st, 0, n, st->d.scratch, q); resident_invalidate(st); }
+    std::vector<char> hcell;
+    if (fresh->cell) {
+        launch_geometry(st, 0, n, st->d.scratch, q);
+        hcell.resize((size_t)n * 9 * (st->d.dtype == TS_F32 ? 4 : 8));
+        TS_CUDA_OK(st, cudaMemcpyAsync(hcell.data(), fresh->cell, hcell.size(), cudaMemcpyDeviceToHost, q));
+    }
     st->list_built = false;
     st->forces_current = false;
     /* the upload buffer must outlive the copy */
     TS_CUDA_OK(st, cudaStreamSynchronize(q));
+    if (fresh->cell) resident_after_swap(st, slots, n, hcell.data());   /* keeps the launch plan when the new cells fit it */
     return check_launch(st);
 }
 

@@ -133,11 +133,17 @@ class InFlightRelaxer:
                 self.peak_resident = max(self.peak_resident, int((slot_id >= 0).sum()))
                 if not done:
                     continue
-                pos = st.numpy("pos")
+                # only the finished systems come back to the host (device-side row selection, then one copy)
+                rows = np.concatenate([np.arange(off[s], off[s + 1]) for s in done])
+                sel = st.torch.from_numpy(rows).to(st.device)
+                pos_done = st.pos.index_select(0, sel).cpu().numpy()
                 energy = st.numpy("energy")
+                at = 0
                 for s in done:
-                    rec = {"pos": pos[off[s]:off[s + 1]].copy(), "energy": float(energy[s]), "fire_steps": int(steps[s]),
+                    n_s = int(off[s + 1] - off[s])
+                    rec = {"pos": pos_done[at:at + n_s].copy(), "energy": float(energy[s]), "fire_steps": int(steps[s]),
                            "status": int(status[s]), "slot": s}
+                    at += n_s
                     sid = int(slot_id[s])
                     self.results[sid] = rec
                     if status[s] == ts.TS_FIRE_CONVERGED:
