@@ -613,18 +613,80 @@ __device__ __forceinline__ unsigned wrap_bit(unsigned uj, unsigned ui)
     return (((~uj & ui) | (~(uj ^ ui) & dd)) ^ dd) >> 31;
 }
 
-__device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, const unsigned *gtab, unsigned short *rows,
+/* shared-memory accesses of the build by 32-bit shared-window address (no generic address arithmetic in the loops) */
+__device__ __forceinline__ uint4 lds_u4(unsigned a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_u16(unsigned a, unsigned v) { asm volatile("st.shared.u16 [%0], %1;" :: "r"(a), "h"((unsigned short)v) : "memory"); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 pk2u(unsigned a, unsigned b)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(a), "r"(b));
+    return r;
+}
+/* u = u_j - u_i + 2^31 (the minimum-image difference of two 32-bit fractions, offset to unsigned) -> the bits of the
+ * float 2^23 + (u >> 9): one funnel shift places the top 23 bits under the exponent of 2^23 (0x4B000000 = 0x96 << 23).
+ * Subtracting 2^23 + 2^22 leaves floor(d / 512), d the signed difference: no integer-to-float conversion (a quarter-rate
+ * instruction: six of them were the limit of the test loop) */
+__device__ __forceinline__ unsigned frac_diff_bits(unsigned u) { return __funnelshift_r(u, 0x96u, 9); }
+
+__device__ __forceinline__ unsigned lds_u8(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+/* bit 31 = 1 when the minimum image of j relative to i along this axis is not the home image (wrap_bit without the shift) */
+__device__ __forceinline__ unsigned wrap_msb(unsigned uj, unsigned ui)
+{
+    const unsigned dd = uj - ui;
+    return ((~uj & ui) | (~(uj ^ ui) & dd)) ^ dd;
+}
+/* entry (act << 3 | mm) of the image-rank table: 8 x the rank of the subset mm among the non-empty subsets of act */
+__device__ __forceinline__ unsigned char image_rank8(int idx)
+{
+    const unsigned act = (unsigned)idx >> 3, mm = (unsigned)idx & 7u;
+    if (mm == 0u || (mm & ~act)) return 0x80;
+    const unsigned a0 = act & 1u, a1 = (act >> 1) & 1u;
+    return (unsigned char)(8u * ((mm & 1u) + (((mm >> 1) & 1u) << a0) + ((mm >> 2) << (a0 + a1)) - 1u));
+}
+
+__device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsigned *gtab, unsigned short *rows,
                                             unsigned *tmeta, const float *G, float rb2, int a_begin, int A_own, int N_s,
-                                            int N8, ResMisc *misc)
+                                            int N8, ResMisc *misc, unsigned rank_sa)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 7, q = lane >> 3;
     const int ntasks = (A_own + 7) >> 3;          /* tasks of the pair phase: eight atoms, built four at a time */
-    const f32x2 G0 = pk2(G[0], G[0]), G1 = pk2(G[1], G[1]), G2 = pk2(G[2], G[2]);
-    const f32x2 G3 = pk2(G[3], G[3]), G4 = pk2(G[4], G[4]), G5 = pk2(G[5], G[5]);
+    /* metric of the fraction differences (units of 2^-23 of the cell): xx, 2xy, 2xz, yy, 2yz, zz.  Orthogonal cell
+     * vectors: the slots of the off-diagonal terms carry l_k = sqrt(G_kk) in G0, G3, G5 and -C l_k in G1, G2, G4 */
+    const bool ortho = G[1] == 0.f && G[2] == 0.f && G[4] == 0.f;
+    const float CF = 12582912.f;                                    /* C = 2^23 + 2^22 */
+    const float l0 = sqrtf(G[0]), l1 = sqrtf(G[3]), l2 = sqrtf(G[5]);
+    const f32x2 G0 = ortho ? pk2(l0, l0) : pk2(G[0], G[0]), G1 = ortho ? pk2(-CF * l0, -CF * l0) : pk2(G[1], G[1]);
+    const f32x2 G2 = ortho ? pk2(-CF * l1, -CF * l1) : pk2(G[2], G[2]), G3 = ortho ? pk2(l1, l1) : pk2(G[3], G[3]);
+    const f32x2 G4 = ortho ? pk2(-CF * l2, -CF * l2) : pk2(G[4], G[4]), G5 = ortho ? pk2(l2, l2) : pk2(G[5], G[5]);
+    const f32x2 NC = pk2(-CF, -CF);
     const bool ovf = misc->overflow != 0;         /* ghost slots exhausted: leave every row empty (flagged) */
     const int T = (N_s + 7) >> 3;                 /* candidates per lane */
     const int W = (T + 31) >> 5;                  /* mask words per lane */
+    const unsigned fr_sa = smem_u32(fr), rows_sa = smem_u32(rows);
+    const unsigned cand_sa = fr_sa + (unsigned)l * 16u;             /* candidate t of lane l: cand_sa + 128 t */
+    /* the gtab entry of every atom rides in the spare word of its fraction: one load per hit in the placement */
+    for (int j = threadIdx.x; j < N_s; j += blockDim.x) {
+        const unsigned e = gtab[j];
+        ((unsigned *)fr)[4 * j + 3] = (e & 0xffffu) | (((e >> 16) & 7u) << 19);   /* first image slot | active axes << 19 */
+    }
+    __syncthreads();
     unsigned nnz = 0;
     for (int task = warp; task < ntasks; task += rc.nwarps) {
       int Rh0 = 0, Rh1 = 0, ai0 = 0;
@@ -634,29 +696,44 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
         const int al = task * 8 + a8;
         const bool has = al < A_own;
         const int ai = hslot(a_begin + (has ? al : 0), N8);     /* slot of the atom: the build works in slot space */
-        const uint4 ui = fr[ai];
+        const uint4 ui = lds_u4(fr_sa + (unsigned)ai * 16u);
+        const unsigned ox = ui.x + 0x80000000u, oy = ui.y + 0x80000000u, oz = ui.z + 0x80000000u;
         unsigned mask[8];
         int mine = 0;
+#ifdef TS_RES_TIMING
+        long long bt0 = clock64();
+#endif
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
             unsigned word = 0u;
             if (w < W) {
-                const uint4 *cj = fr + (w * 256 + l);
+                const unsigned cw = cand_sa + (unsigned)w * 4096u;
                 const int nb = min(32, T - w * 32);                 /* uniform */
 #pragma unroll 4
                 for (int b = 0; b < nb; b += 2) {
-                    const uint4 ua = cj[b * 8], ub = cj[b * 8 + 8];
-                    const f32x2 E0 = pk2((float)(int)(ua.x - ui.x), (float)(int)(ub.x - ui.x));
-                    const f32x2 E1 = pk2((float)(int)(ua.y - ui.y), (float)(int)(ub.y - ui.y));
-                    const f32x2 E2 = pk2((float)(int)(ua.z - ui.z), (float)(int)(ub.z - ui.z));
-                    f32x2 A0 = mul2(G0, E0);
-                    A0 = fma2(G1, E1, A0);
-                    A0 = fma2(G2, E2, A0);
-                    f32x2 A1 = mul2(G3, E1);
-                    A1 = fma2(G4, E2, A1);
-                    f32x2 R = mul2(mul2(G5, E2), E2);
-                    R = fma2(E1, A1, R);
-                    R = fma2(E0, A0, R);
+                    const uint4 ua = lds_u4(cw + (unsigned)b * 128u), ub = lds_u4(cw + (unsigned)b * 128u + 128u);
+                    const f32x2 F0 = pk2u(frac_diff_bits(ua.x - ox), frac_diff_bits(ub.x - ox));
+                    const f32x2 F1 = pk2u(frac_diff_bits(ua.y - oy), frac_diff_bits(ub.y - oy));
+                    const f32x2 F2 = pk2u(frac_diff_bits(ua.z - oz), frac_diff_bits(ub.z - oz));
+                    f32x2 R;
+                    if (ortho) {
+                        /* orthogonal cell vectors: Cartesian components l_k (F_k - C) straight from the bits, the offset
+                         * folded into the product (its rounding shifts every difference vector by the same < 1e-7 L) */
+                        const f32x2 Y0 = fma2(F0, G0, G1), Y1 = fma2(F1, G3, G2), Y2 = fma2(F2, G5, G4);
+                        R = mul2(Y0, Y0);
+                        R = fma2(Y1, Y1, R);
+                        R = fma2(Y2, Y2, R);
+                    } else {
+                        const f32x2 E0 = add2(F0, NC), E1 = add2(F1, NC), E2 = add2(F2, NC);
+                        f32x2 A0 = mul2(G0, E0);
+                        A0 = fma2(G1, E1, A0);
+                        A0 = fma2(G2, E2, A0);
+                        f32x2 A1 = mul2(G3, E1);
+                        A1 = fma2(G4, E2, A1);
+                        R = mul2(mul2(G5, E2), E2);
+                        R = fma2(E1, A1, R);
+                        R = fma2(E0, A0, R);
+                    }
                     float ra, rb;
                     upk2(R, ra, rb);
                     if (ra < rb2) word |= 1u << b;
@@ -672,6 +749,9 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
             mask[w] = word;
             mine += __popc(word);
         }
+#ifdef TS_RES_TIMING
+        if (threadIdx.x == 0) { long long t = clock64(); atomicAdd(&g_res_prof[12], (unsigned long long)(t - bt0)); bt0 = t; }
+#endif
         /* entries of the lanes below (exclusive prefix inside the quarter-warp) and of the whole atom */
         int inc = mine;
 #pragma unroll
@@ -680,9 +760,6 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
             if (l >= o) inc += v;
         }
         const int NT = __shfl_sync(0xffffffffu, inc, 7, 8);
-        int cq[8];                                                    /* populations of the eight bank groups of the atom */
-#pragma unroll
-        for (int c = 0; c < 8; ++c) cq[c] = __shfl_sync(0xffffffffu, mine, c, 8);
         int R = ((NT + 15) >> 4) << 1;                                /* rows: whole trips of 16 entries */
         R = max(R, __shfl_xor_sync(0xffffffffu, R, 8));
         R = max(R, __shfl_xor_sync(0xffffffffu, R, 16));              /* the four atoms of a half task place into the same rows */
@@ -694,10 +771,10 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
         /* u16 halves of the trip words of this atom (see "list layout"): row r of column c lives at
          * base + (r / 2) * 128 + (c & 3) * 4 + (r & 1) * 2 + ((c >> 2) ^ p), p = parity of the atom in its task;
          * the odd half holds the entry << 2 (bits 18..31 of the word) */
-        unsigned short *rowB = rows + (size_t)task * rc.pitch * 8 + a8 * 16;
         const int par = a8 & 1;
-#define CELL_B(r, c) rowB[((r) >> 1) * 128 + ((c) & 3) * 4 + ((r) & 1) * 2 + (((c) >> 2) ^ par)]
-#define ENT(slot, c) (unsigned short)((unsigned)(slot) << (((((c) >> 2) ^ par)) << 1))
+        const unsigned rowB_sa = rows_sa + 2u * ((unsigned)task * (unsigned)rc.pitch * 8u + (unsigned)a8 * 16u);
+#define CELL_SA(r, c) (rowB_sa + 2u * (unsigned)(((r) >> 1) * 128 + ((c) & 3) * 4 + ((r) & 1) * 2 + (((c) >> 2) ^ par)))
+#define ENT(slot, c) ((unsigned)(slot) << (((((c) >> 2) ^ par)) << 1))
         if (fits) {
             /* Placement.  The pair loop reads R rows of eight entries; entry (row, column) is read by lane
              * `column`, and one shared-memory wavefront serves a row when its eight bank groups differ.  Lane l
@@ -716,47 +793,74 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
             const int F_l = jf - f_l;                                     /* free cells in the columns below l */
             const int recv = min(max(O - F_l, 0), f_l);                   /* overflow entries that land in column l */
             int u = io - o_l;                                             /* number of my first overflow entry */
-            int m = 0;
+            /* slot of the neighbour whose fraction lies at shared address ja, as seen from atom i: its home slot, or the
+             * slot of the image the minimum-image convention selects (bit k of mm: the pair wraps along axis k) */
+            auto slot_of = [&](unsigned ja, unsigned j) -> unsigned {
+                const uint4 uj = lds_u4(ja);
+                /* mm = wrap bits of z, y, x: three funnel shifts collect the three top bits */
+                const unsigned mm = __funnelshift_l(wrap_msb(uj.x, ui.x), __funnelshift_l(wrap_msb(uj.y, ui.y), wrap_msb(uj.z, ui.z) >> 31, 1), 1);
+                unsigned slot = j;
+                if (mm) {
+                    /* uj.w = first image slot | active axes << 19: the byte table gives 8 x the rank of the subset mm among
+                     * the non-empty subsets of the active axes (0x80: not a subset -- cannot happen, see ghost_table) */
+                    const unsigned r8 = lds_u8(rank_sa + (uj.w >> 16) + mm);
+                    if (r8 & 0x80u) misc->overflow = 1;
+                    slot = (uj.w & 0xffffu) + r8;
+                }
+                return slot;
+            };
+            /* pass 1: the first R hits of the lane go down its own column -- the common case, kept lean */
+            const unsigned cmul = 1u << ((((l >> 2) ^ par)) << 1);        /* the odd half holds the entry << 2 */
+            unsigned cell = CELL_SA(0, l), dlt = 4u;
+            int left = R;
 #pragma unroll
             for (int w = 0; w < 8; ++w) {
                 unsigned word = mask[w];
-                while (word) {
-                    const int b = __ffs(word) - 1;
+                const unsigned cw = cand_sa + (unsigned)w * 4096u, jw = (unsigned)(w * 256 + l);
+                while (word && left) {
+                    const unsigned b = (unsigned)__ffs(word) - 1u;
                     word &= word - 1u;
-                    const int j = ((w * 32 + b) << 3) + l;
-                    const uint4 uj = fr[j];
-                    const unsigned mm = wrap_bit(uj.x, ui.x) | (wrap_bit(uj.y, ui.y) << 1) | (wrap_bit(uj.z, ui.z) << 2);
-                    unsigned slot = (unsigned)j;
-                    if (mm) {
-                        const unsigned gd = gtab[j];
-                        const unsigned a0 = (gd >> 16) & 1u, a1 = (gd >> 17) & 1u;
-                        /* rank of the subset mm among the non-empty subsets of the active axes */
-                        const unsigned r = (mm & 1u) + (((mm >> 1) & 1u) << a0) + ((mm >> 2) << (a0 + a1)) - 1u;
-                        if ((mm & ~(gd >> 16)) & 7u) misc->overflow = 1;                  /* cannot happen: see ghost_table */
-                        slot = (gd & 0xffffu) + 8u * r;
-                    }
-                    int prow = m, pcol = l;
-                    if (m >= R) {                                          /* the u-th free cell, column-major */
-                        int P = 0, Fc = 0;
-                        pcol = 0;
+                    sts_u16(cell, slot_of(cw + b * 128u, jw + b * 8u) * cmul);
+                    cell += dlt;                                       /* row m + 1 of the column: + 4, + 252, + 4, ... bytes */
+                    dlt = 256u - dlt;
+                    --left;
+                }
+                mask[w] = word;
+            }
+            /* pass 2: the overflow hits (what is left in the masks) take the free cells, column-major */
+            int cq[8];                                                    /* populations of the eight bank groups of the atom */
 #pragma unroll
-                        for (int c = 0; c < 8; ++c) {                      /* columns whose free cells all come before cell u */
-                            P += R - min(R, cq[c]);
-                            if (P <= u) { pcol = c + 1; Fc = P; }
-                        }
-                        int cc = 0;
+            for (int c = 0; c < 8; ++c) cq[c] = __shfl_sync(0xffffffffu, mine, c, 8);
+#pragma unroll 1
+            for (int w = 0; w < W; ++w) {
+                unsigned word = mask[0];
 #pragma unroll
-                        for (int c = 0; c < 8; ++c) cc = pcol == c ? cq[c] : cc;
-                        prow = cc + (u - Fc);
-                        ++u;
+                for (int k = 1; k < 8; ++k) word = w == k ? mask[k] : word;
+                const unsigned cw = cand_sa + (unsigned)w * 4096u, jw = (unsigned)(w * 256 + l);
+                while (word) {
+                    const unsigned b = (unsigned)__ffs(word) - 1u;
+                    word &= word - 1u;
+                    const unsigned slot = slot_of(cw + b * 128u, jw + b * 8u);
+                    int P = 0, Fc = 0, pcol = 0;
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {                      /* columns whose free cells all come before cell u */
+                        P += R - min(R, cq[c]);
+                        if (P <= u) { pcol = c + 1; Fc = P; }
                     }
-                    CELL_B(prow, pcol) = ENT(slot, pcol);
-                    ++m;
+                    int cc = 0;
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) cc = pcol == c ? cq[c] : cc;
+                    const int prow = cc + (u - Fc);
+                    ++u;
+                    sts_u16(CELL_SA(prow, pcol), ENT(slot, pcol));
                 }
             }
             /* padding of my column below my own hits and the overflow entries it received */
-            for (int r = min(mine, R) + recv; r < R; ++r) CELL_B(r, l) = ENT(N8 + l, l);
+            for (int r = min(mine, R) + recv; r < R; ++r) sts_u16(CELL_SA(r, l), ENT(N8 + l, l));
         }
+#ifdef TS_RES_TIMING
+        if (threadIdx.x == 0) { long long t = clock64(); atomicAdd(&g_res_prof[13], (unsigned long long)(t - bt0)); bt0 = t; }
+#endif
         if (half == 0) { Rh0 = R; ai0 = has ? ai : N8; } else Rh1 = R;
         if (has) nnz += (unsigned)mine;
         if (half == 1) {
@@ -766,13 +870,13 @@ __device__ __forceinline__ void build_phase(const ResCfg &rc, const uint4 *fr, c
             const int par0 = q & 1;
             for (int r = Rh0; r < Rm; ++r)
                 row0[(r >> 1) * 128 + (l & 3) * 4 + (r & 1) * 2 + ((l >> 2) ^ par0)] = (unsigned short)((unsigned)(N8 + l) << (((l >> 2) ^ par0) << 1));
-            for (int r = Rh1; r < Rm; ++r) CELL_B(r, l) = ENT(N8 + l, l);
+            for (int r = Rh1; r < Rm; ++r) sts_u16(CELL_SA(r, l), ENT(N8 + l, l));
             if (l == 0) {
                 tmeta[task * 8 + q] = (unsigned)ai0 | ((unsigned)(Rm >> 1) << 14);
                 tmeta[task * 8 + 4 + q] = (unsigned)(has ? ai : N8) | ((unsigned)(Rm >> 1) << 14);
             }
         }
-#undef CELL_B
+#undef CELL_SA
 #undef ENT
       }
     }
@@ -890,6 +994,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     }
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
+    __shared__ unsigned char s_rank[64];          /* image-rank table of the list build */
+    if (tid < 64) s_rank[tid] = image_rank8(tid);
 
     for (int ks = cid; ks < rc.n_list; ks += rc.n_clusters) {
         const int s = rc.syslist ? rc.syslist[ks] : ks;
@@ -920,7 +1026,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 M[e] = h[3 * a] * h[3 * b] + h[3 * a + 1] * h[3 * b + 1] + h[3 * a + 2] * h[3 * b + 2];
                 if (a != b) M[e] *= 2.0;
             }
-            const double sc = 1.0 / 18446744073709551616.0;      /* 2^-64 */
+            const double sc = 1.0 / 70368744177664.0;            /* 2^-46: the build measures fractions in units of 2^-23 */
             for (int e = 0; e < 6; ++e) G[e] = (float)(M[e] * sc);
             for (int a = 0; a < 3; ++a) lmax = fmax(lmax, sqrt(h[3 * a] * h[3 * a] + h[3 * a + 1] * h[3 * a + 1] + h[3 * a + 2] * h[3 * a + 2]));
             const double rb = d.r_list + (double)rc.eps_rel * lmax;
@@ -1107,7 +1213,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 TICK(5);
                 ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
                 TICK(6);
-                build_phase(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc);
+                build_phase(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc, smem_u32(s_rank));
                 __syncthreads();
                 TICK(7);
                 ghost_pass<T>(posb, zt, gtab, gh, N_s);          /* images again: the rebuild re-wrapped the home slots */
