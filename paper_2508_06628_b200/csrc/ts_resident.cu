@@ -639,6 +639,13 @@ __device__ __forceinline__ f32x2 pk2u(unsigned a, unsigned b)
  * instruction: six of them were the limit of the test loop) */
 __device__ __forceinline__ unsigned frac_diff_bits(unsigned u) { return __funnelshift_r(u, 0x96u, 9); }
 
+/* all ones when a < b, else zero */
+__device__ __forceinline__ unsigned set_lt(float a, float b)
+{
+    unsigned r;
+    asm("set.lt.u32.f32 %0, %1, %2;" : "=r"(r) : "f"(a), "f"(b));
+    return r;
+}
 __device__ __forceinline__ unsigned lds_u8(unsigned a)
 {
     unsigned v;
@@ -660,6 +667,7 @@ __device__ __forceinline__ unsigned char image_rank8(int idx)
     return (unsigned char)(8u * ((mm & 1u) + (((mm >> 1) & 1u) << a0) + ((mm >> 2) << (a0 + a1)) - 1u));
 }
 
+template <bool ORTHO>
 __device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsigned *gtab, unsigned short *rows,
                                             unsigned *tmeta, const float *G, float rb2, int a_begin, int A_own, int N_s,
                                             int N8, ResMisc *misc, unsigned rank_sa)
@@ -669,7 +677,7 @@ __device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsi
     const int ntasks = (A_own + 7) >> 3;          /* tasks of the pair phase: eight atoms, built four at a time */
     /* metric of the fraction differences (units of 2^-23 of the cell): xx, 2xy, 2xz, yy, 2yz, zz.  Orthogonal cell
      * vectors: the slots of the off-diagonal terms carry l_k = sqrt(G_kk) in G0, G3, G5 and -C l_k in G1, G2, G4 */
-    const bool ortho = G[1] == 0.f && G[2] == 0.f && G[4] == 0.f;
+    const bool ortho = ORTHO;
     const float CF = 12582912.f;                                    /* C = 2^23 + 2^22 */
     const float l0 = sqrtf(G[0]), l1 = sqrtf(G[3]), l2 = sqrtf(G[5]);
     const f32x2 G0 = ortho ? pk2(l0, l0) : pk2(G[0], G[0]), G1 = ortho ? pk2(-CF * l0, -CF * l0) : pk2(G[1], G[1]);
@@ -716,7 +724,7 @@ __device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsi
                     const f32x2 F1 = pk2u(frac_diff_bits(ua.y - oy), frac_diff_bits(ub.y - oy));
                     const f32x2 F2 = pk2u(frac_diff_bits(ua.z - oz), frac_diff_bits(ub.z - oz));
                     f32x2 R;
-                    if (ortho) {
+                    if (ORTHO) {
                         /* orthogonal cell vectors: Cartesian components l_k (F_k - C) straight from the bits, the offset
                          * folded into the product (its rounding shifts every difference vector by the same < 1e-7 L) */
                         const f32x2 Y0 = fma2(F0, G0, G1), Y1 = fma2(F1, G3, G2), Y2 = fma2(F2, G5, G4);
@@ -736,9 +744,11 @@ __device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsi
                     }
                     float ra, rb;
                     upk2(R, ra, rb);
-                    if (ra < rb2) word |= 1u << b;
-                    if (rb < rb2) word |= 2u << b;
+                    /* the hit bits enter at the top and move down: candidate 0 of the word ends up in bit 0 */
+                    word = __funnelshift_r(word, set_lt(ra, rb2), 1);
+                    word = __funnelshift_r(word, set_lt(rb, rb2), 1);
                 }
+                if (nb < 31) word >>= 32 - ((nb + 1) & ~1);        /* the loop tests candidates in pairs */
                 /* candidates past the end of the system (padding) and the atom itself */
                 const int tmax = (N_s - l + 7) >> 3;                /* lane l owns t < tmax */
                 const int keep = tmax - w * 32;
@@ -1213,7 +1223,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                 TICK(5);
                 ghost_table(rc, fr, gtab, thr, N_s, N8 + 8, misc);
                 TICK(6);
-                build_phase(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc, smem_u32(s_rank));
+                if (G[1] == 0.f && G[2] == 0.f && G[4] == 0.f) build_phase<true>(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc, smem_u32(s_rank));
+                else build_phase<false>(rc, fr, gtab, rows, tmeta, G, G[6], a_begin, A_own, N_s, N8, misc, smem_u32(s_rank));
                 __syncthreads();
                 TICK(7);
                 ghost_pass<T>(posb, zt, gtab, gh, N_s);          /* images again: the rebuild re-wrapped the home slots */
