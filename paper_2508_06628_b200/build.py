@@ -30,6 +30,11 @@ def _stale(out, deps):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    # objects compiled with other flags (a debugging define) are stale whatever their age
+    stamp = os.path.join(OBJ, "flags.txt")
+    flags = " ".join(FLAGS)
+    if not os.path.exists(stamp) or open(stamp).read() != flags:
+        force = True
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(ROOT, "include", "ts.h"))
     jobs = []
@@ -52,6 +57,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
     if force or jobs or _stale(LIB, objs):
         run([NVCC, "-shared", "-o", LIB] + objs)
+    with open(stamp, "w") as f:
+        f.write(flags)
     return LIB
 
 
