@@ -231,6 +231,24 @@ ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int64_t *off, 
 ts_status ts_export_edges(ts_state *st, int64_t *edge_i, int64_t *edge_j, void *edge_shift, int64_t cap,
                           int64_t *n_edges, void *stream);
 
+/* ts_export_edges for callers that must not allocate and cannot lend workspace scratch (code under CUDA graph
+ * capture, tight serving loops): same arguments, same result, but the per-system exclusive scan of the edge counts
+ * lives in a file-scope device array of the library instead of a workspace region.  No cudaMalloc / cudaFree or
+ * allocating library routine is called (no entry point of this library allocates device memory; this one also
+ * borrows none from the workspace for its scratch).
+ *   limit      at most 16,384 systems in the state (the array holds 16,385 int64 = 131,080 bytes on every GPU that
+ *              loads the library, until the process exits); more: TS_ERR_WORKSPACE_TOO_SMALL, ts_last_error names
+ *              the limit, nothing is launched, use ts_export_edges.
+ *   sharing    ONE array per GPU, shared by every state and every call; it keeps the contents of the last call.  Each
+ *              call rewrites the entries it reads before reading them, so nothing needs clearing -- but two calls that
+ *              overlap on the GPU (different streams, no ordering between them) race on it and give wrong edges.
+ *   set-up     the device address of the array is looked up once per device on the first call with that device
+ *              current; ts_static_scratch_setup does the same ahead of time (call it before a stream capture starts).
+ * ts_static_scratch_setup: *max_systems (host, may be NULL) = the limit; TS_ERR_CUDA if the lookup fails.            */
+ts_status ts_export_edges_static(ts_state *st, int64_t *edge_i, int64_t *edge_j, void *edge_shift, int64_t cap,
+                                 int64_t *n_edges, void *stream);
+ts_status ts_static_scratch_setup(int64_t *max_systems);
+
 /* One MD / FIRE step split around a force evaluation the CALLER enqueues on `stream` (an external energies / forces /
  * stress provider writing desc.force, and desc.energy / desc.virial if it wants them reported):
  *   MD:   TS_PHASE_INIT (list for the current positions) -> caller: F(x) -> then per step

@@ -32,7 +32,7 @@ EXPORTS = ["ts_workspace_bytes", "ts_estimate_system_bytes", "ts_state_create", 
            "ts_status_string", "ts_last_error", "ts_sched_fill", "ts_sched_max_scaler",
            "ts_sched_binpack", "ts_sched_partition", "ts_repack_systems", "ts_get_capacity",
            "ts_estimate_system_pairs", "ts_export_edges", "ts_md_step_external", "ts_fire_step_external",
-           "ts_measure_fma_tflops", "ts_get_resident_neighbors"]
+           "ts_measure_fma_tflops", "ts_get_resident_neighbors", "ts_export_edges_static", "ts_static_scratch_setup"]
 
 TS_PHASE_INIT, TS_PHASE_PRE, TS_PHASE_POST, TS_PHASE_CHECK0 = 0, 1, 2, 3
 (TS_OK, TS_ERR_INVALID_ARG, TS_ERR_CUDA, TS_ERR_WORKSPACE_TOO_SMALL, TS_ERR_NBR_OVERFLOW, TS_ERR_STALE_NBR,
@@ -209,6 +209,18 @@ def ts_estimate_system_pairs(n_atoms, volume, r_list, slack=1.25):
 def ts_export_edges(h, edge_i_ptr, edge_j_ptr, edge_shift_ptr, cap, n_edges_ptr):
     _check(lib().ts_export_edges(h, C.c_void_p(edge_i_ptr), C.c_void_p(edge_j_ptr), C.c_void_p(edge_shift_ptr),
                                  C.c_int64(cap), C.c_void_p(n_edges_ptr), _stream()), "ts_export_edges", h)
+
+
+def ts_export_edges_static(h, edge_i_ptr, edge_j_ptr, edge_shift_ptr, cap, n_edges_ptr):
+    _check(lib().ts_export_edges_static(h, C.c_void_p(edge_i_ptr), C.c_void_p(edge_j_ptr), C.c_void_p(edge_shift_ptr),
+                                        C.c_int64(cap), C.c_void_p(n_edges_ptr), _stream()), "ts_export_edges_static", h)
+
+
+def ts_static_scratch_setup():
+    """Looks up the library's static scratch array on the current device; returns its limit in systems."""
+    n = C.c_int64(0)
+    _check(lib().ts_static_scratch_setup(C.byref(n)), "ts_static_scratch_setup")
+    return int(n.value)
 
 
 def ts_md_step_external(h, params, phase):

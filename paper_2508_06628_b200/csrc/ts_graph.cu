@@ -2,6 +2,7 @@
  * ts_graph.cu -- the batched graph builder as a service to an external energies / forces / stress
  * provider (SURVEY.md 8(f) NEXT-2; PAPER.md:56 "ModelInterface", :112 "graph construction"):
  *   ts_export_edges          the current Verlet list as a dense device-side edge list (i, j, S)
+ *   ts_export_edges_static   the same with its scratch in a file-scope device array (no workspace region, no allocation)
  *   ts_md_step_external      one MD step split around a force evaluation the caller does
  *   ts_fire_step_external    the same for FIRE
  * The integrators are the general engine's kernels, unchanged; only the pair kernel is replaced by
@@ -9,6 +10,8 @@
  */
 #include <math.h>
 #include <string.h>
+
+#include <mutex>
 
 #include "ts_internal.cuh"
 
@@ -85,6 +88,71 @@ extern "C" ts_status ts_export_edges(ts_state *st, int64_t *edge_i, int64_t *edg
     else k_edge_fill<double><<<nb, 256, 0, q>>>(d, edge_base, (long long *)edge_i, (long long *)edge_j, (double *)edge_shift, cap);
     st->launches += 2;
     cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { ts_set_error(st, "edge export failed: %s", cudaGetErrorString(e)); return TS_ERR_CUDA; }
+    return TS_OK;
+}
+
+/* ------------------------------------------------------------------ edge export without workspace scratch
+ * ts_export_edges keeps its [S + 1] exclusive scan of the edge counts in a workspace region the next list build
+ * rewrites.  The variant below keeps it in a file-scope device array instead, for callers that must not allocate and
+ * whose workspace region is in use: every GPU that loads the library holds the array (131,080 bytes) until exit.
+ * In host code `g_edge_scan` is only a stand-in for the symbol, not a device address: the address the kernels get is
+ * looked up with cudaGetSymbolAddress once per device, with that device current.                                     */
+#define TS_STATIC_EDGE_MAX_SYSTEMS 16384
+#define TS_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) long long g_edge_scan[TS_STATIC_EDGE_MAX_SYSTEMS + 1];
+
+static std::mutex g_edge_scan_lock;
+static long long *g_edge_scan_addr[TS_STATIC_MAX_DEVICES];      /* device address of g_edge_scan, by device ordinal */
+
+/* address of the array on the CURRENT device (looked up on the first call for that device); nullptr + *err on failure */
+static long long *edge_scan_address(cudaError_t *err)
+{
+    int dev = -1;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= TS_STATIC_MAX_DEVICES) { *err = cudaErrorInvalidDevice; return nullptr; }
+    std::lock_guard<std::mutex> hold(g_edge_scan_lock);
+    if (!g_edge_scan_addr[dev]) {
+        long long *p = nullptr;
+        *err = cudaGetSymbolAddress((void **)&p, g_edge_scan);
+        if (*err != cudaSuccess) return nullptr;
+        g_edge_scan_addr[dev] = p;
+    }
+    return g_edge_scan_addr[dev];
+}
+
+extern "C" ts_status ts_static_scratch_setup(int64_t *max_systems)
+{
+    if (max_systems) *max_systems = TS_STATIC_EDGE_MAX_SYSTEMS;
+    cudaError_t e = cudaSuccess;
+    return edge_scan_address(&e) ? TS_OK : TS_ERR_CUDA;
+}
+
+extern "C" ts_status ts_export_edges_static(ts_state *st, int64_t *edge_i, int64_t *edge_j, void *edge_shift, int64_t cap,
+                                            int64_t *n_edges, void *stream)
+{
+    if (!st || !edge_i || !edge_j || !edge_shift || !n_edges || cap < 0) return TS_ERR_INVALID_ARG;
+    if (st->seen_flags) return TS_ERR_STICKY;
+    if (st->d.S > TS_STATIC_EDGE_MAX_SYSTEMS) {
+        ts_set_error(st, "ts_export_edges_static: %d systems, the static scratch array holds at most %d (use ts_export_edges)",
+                     st->d.S, TS_STATIC_EDGE_MAX_SYSTEMS);
+        return TS_ERR_WORKSPACE_TOO_SMALL;
+    }
+    cudaError_t e = cudaSuccess;
+    long long *edge_base = edge_scan_address(&e);
+    if (!edge_base) { ts_set_error(st, "address of the static scratch array: %s", cudaGetErrorString(e)); return TS_ERR_CUDA; }
+    cudaStream_t q = (cudaStream_t)stream;
+    ensure_list_graph(st, q);
+    const DevState &d = st->d;
+    /* the array keeps what the last call left: k_edge_base rewrites entries 0 .. S before k_edge_fill reads them, and
+     * nothing is accumulated into it, so nothing has to be cleared */
+    k_edge_base<<<1, 256, 0, q>>>(d, edge_base, (long long *)n_edges);
+    const unsigned nb = (unsigned)((d.N * 8 + 255) / 256);
+    if (d.dtype == TS_F32) k_edge_fill<float><<<nb, 256, 0, q>>>(d, edge_base, (long long *)edge_i, (long long *)edge_j, (float *)edge_shift, cap);
+    else k_edge_fill<double><<<nb, 256, 0, q>>>(d, edge_base, (long long *)edge_i, (long long *)edge_j, (double *)edge_shift, cap);
+    st->launches += 2;
+    e = cudaGetLastError();
     if (e != cudaSuccess) { ts_set_error(st, "edge export failed: %s", cudaGetErrorString(e)); return TS_ERR_CUDA; }
     return TS_OK;
 }

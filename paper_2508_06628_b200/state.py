@@ -210,6 +210,12 @@ class SimState:
             raise ts.TsError(ts.TS_ERR_WORKSPACE_TOO_SMALL, "export_edges", f"{n} edges > capacity {ei.shape[1]}")
         return ei[:, :n], es[:n]
 
+    def export_edges_static(self, edge_index, edge_shift, n_edges):
+        """ts_export_edges_static into the CALLER's device tensors (edge_index [2, cap] int64, edge_shift [cap, 3] in
+        the state dtype, n_edges [1] int64): no allocation, no read-back; scratch in the library's static array."""
+        ts.ts_export_edges_static(self.handle, edge_index[0].data_ptr(), edge_index[1].data_ptr(), edge_shift.data_ptr(),
+                                  edge_index.shape[1], n_edges.data_ptr())
+
     def md_step_external(self, params, phase):
         if isinstance(params, dict):
             params = ts.md_params(**params)
