@@ -182,6 +182,14 @@ ts_status ts_poll(ts_state *st, ts_report *out, void *stream);
 ts_status ts_converged_mask(ts_state *st, uint8_t *mask, int32_t *status, int32_t *fire_steps,
                             void *stream);
 
+/* The same status words WITHOUT synchronising: status[s] and fire_steps[s] (HOST arrays of S int32, either may be
+ * NULL) are filled by copies enqueued on `stream` behind the work already there; they are valid once the caller has
+ * waited for that point of the stream (an event recorded after this call).  The arrays should be page-locked
+ * (cudaHostAlloc / a pinned torch tensor): with pageable memory CUDA falls back to a copy that blocks the host.
+ * Lets an in-flight scheduler enqueue the next ts_fire_step before it has read the result of the last one: systems
+ * that converged meanwhile stay bit-unchanged (R22), so acting on a status that is one call old changes no result. */
+ts_status ts_fire_status_async(ts_state *st, int32_t *status, int32_t *fire_steps, void *stream);
+
 /* In-flight swap, equal sizes (ts_repack_systems: any sizes).  Synchronises `stream`; the
  * stepping call that follows a swap with new cells re-plans the resident engine (one small device read).
  * Replaces the systems in `slots` (HOST, n entries) by the

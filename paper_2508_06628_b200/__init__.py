@@ -32,7 +32,8 @@ EXPORTS = ["ts_workspace_bytes", "ts_estimate_system_bytes", "ts_state_create", 
            "ts_status_string", "ts_last_error", "ts_sched_fill", "ts_sched_max_scaler",
            "ts_sched_binpack", "ts_sched_partition", "ts_repack_systems", "ts_get_capacity",
            "ts_estimate_system_pairs", "ts_export_edges", "ts_md_step_external", "ts_fire_step_external",
-           "ts_measure_fma_tflops", "ts_get_resident_neighbors", "ts_export_edges_static", "ts_static_scratch_setup"]
+           "ts_measure_fma_tflops", "ts_get_resident_neighbors", "ts_export_edges_static", "ts_static_scratch_setup",
+           "ts_fire_status_async"]
 
 TS_PHASE_INIT, TS_PHASE_PRE, TS_PHASE_POST, TS_PHASE_CHECK0 = 0, 1, 2, 3
 (TS_OK, TS_ERR_INVALID_ARG, TS_ERR_CUDA, TS_ERR_WORKSPACE_TOO_SMALL, TS_ERR_NBR_OVERFLOW, TS_ERR_STALE_NBR,
@@ -177,6 +178,11 @@ def ts_converged_mask(h, n_systems):
     _check(lib().ts_converged_mask(h, mask.ctypes.data_as(C.c_void_p), status.ctypes.data_as(C.c_void_p),
                                    steps.ctypes.data_as(C.c_void_p), _stream()), "ts_converged_mask", h)
     return mask.astype(bool), status, steps
+
+
+def ts_fire_status_async(h, status_ptr, steps_ptr):
+    """status_ptr / steps_ptr: addresses of page-locked HOST int32 arrays of S entries (0 = skip)."""
+    _check(lib().ts_fire_status_async(h, C.c_void_p(status_ptr), C.c_void_p(steps_ptr), _stream()), "ts_fire_status_async", h)
 
 
 def ts_swap_systems(h, slots, fresh_desc):

@@ -211,6 +211,16 @@ extern "C" ts_status ts_converged_mask(ts_state *st, uint8_t *mask, int32_t *sta
     return TS_OK;
 }
 
+extern "C" ts_status ts_fire_status_async(ts_state *st, int32_t *status, int32_t *fire_steps, void *stream)
+{
+    if (!st) return TS_ERR_INVALID_ARG;
+    const size_t bytes = sizeof(int) * (size_t)st->d.S;
+    cudaStream_t q = (cudaStream_t)stream;
+    if (status) TS_CUDA_OK(st, cudaMemcpyAsync(status, st->d.f_status, bytes, cudaMemcpyDeviceToHost, q));
+    if (fire_steps) TS_CUDA_OK(st, cudaMemcpyAsync(fire_steps, st->d.f_nsteps, bytes, cudaMemcpyDeviceToHost, q));
+    return TS_OK;
+}
+
 extern "C" ts_status ts_swap_systems(ts_state *st, const int32_t *slots, int32_t n, const ts_state_desc *fresh, void *stream)
 {
     NEED_STATE(st);

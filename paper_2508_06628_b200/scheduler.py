@@ -98,8 +98,9 @@ class InFlightRelaxer:
     """
 
     def __init__(self, make_batch, n_total, fire, n_slots=None, budget_bytes=None, k_check=10, device="cuda:0",
-                 engine=None, slack=1.25):
+                 engine=None, slack=1.25, pipelined=True):
         self.make_batch, self.n_total, self.fire, self.k_check = make_batch, int(n_total), dict(fire), int(k_check)
+        self.pipelined = bool(pipelined)
         probe = make_batch([0])
         self.bytes_per_system = float(batch_system_bytes(probe, slack)[0])
         if n_slots is None:
@@ -115,6 +116,100 @@ class InFlightRelaxer:
         self.peak_resident = 0
 
     def run(self, target=None, max_rounds=100000):
+        if self.pipelined:
+            return self._run_pipelined(target, max_rounds)
+        return self._run_blocking(target, max_rounds)
+
+    def _run_pipelined(self, target, max_rounds):
+        """The same schedule with the device kept busy: ts_fire_step number r is enqueued BEFORE the status of call
+        r - 1 is read (ts_fire_status_async into page-locked buffers, one event per call), and everything the host does
+        with that status -- picking the finished systems, cutting the fresh ones from the stream, staging their upload --
+        runs while call r computes.  A system that had converged in call r - 1 is frozen in call r (R22), and a slot
+        refilled during round r is ignored in the stale snapshot of call r, so every id ends exactly as in the blocking
+        loop; only the round in which a slot is refilled moves by one."""
+        from .state import SimState
+        target = self.n_total if target is None else int(target)
+        ids = list(range(self.n_slots))
+        next_id = self.n_slots
+        b = self.make_batch(ids)
+        st = SimState(b, device=self.device, engine=self.engine, slack=self.slack)
+        torch = st.torch
+        off = np.asarray(b.sys_offset).astype(np.int64)
+        n_s = int(off[1] - off[0])
+        S = self.n_slots
+        slot_id = np.array(ids, dtype=np.int64)          # stream id resident in each slot, -1 = idle
+        valid_from = np.zeros(S, dtype=np.int64)         # first call whose status describes the system now in the slot
+        fp = ts.fire_params(**self.fire)
+        pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory()
+        snaps = [(pin((S,), torch.int32), pin((S,), torch.int32), torch.cuda.Event()) for _ in range(2)]
+        stage = st.pinned_stage(S * n_s, S)
+        pos_host, energy_host, sel_host = pin((S * n_s, 3), st.tdtype), pin((S,), torch.float64), pin((S * n_s,), torch.int64)
+        lane = np.arange(n_s, dtype=np.int64)
+        n_done = 0
+        stream = torch.cuda.current_stream()
+
+        def harvest(q):
+            """Act on the status of call q (call q + 1 is already enqueued).  True when the run is over."""
+            nonlocal n_done, next_id
+            status_t, steps_t, ev = snaps[q % 2]
+            ev.synchronize()
+            status, steps = status_t.numpy(), steps_t.numpy()
+            fin = (status == ts.TS_FIRE_CONVERGED) | (status == ts.TS_FIRE_FAILED)
+            done = np.nonzero((slot_id >= 0) & (valid_from <= q) & fin)[0]
+            self.peak_resident = max(self.peak_resident, int((slot_id >= 0).sum()))
+            if done.size == 0:
+                return False
+            m = done.size * n_s
+            # host work first (the device is stepping): row numbers of the finished systems, the fresh batch, its staging
+            sel_host[:m].copy_(torch.from_numpy((off[done][:, None] + lane[None, :]).reshape(-1)))
+            n_conv = int((status[done] == ts.TS_FIRE_CONVERGED).sum())
+            take = 0 if n_done + n_conv >= target else min(done.size, self.n_total - next_id)
+            new_ids = list(range(next_id, next_id + take))
+            fresh = self.make_batch(new_ids) if take > 0 else None
+            # enqueued behind the running call: the finished systems (frozen, so unchanged by that call) come back ...
+            sel = sel_host[:m].to(st.device, non_blocking=True)
+            pos_host[:m].copy_(st.pos.index_select(0, sel), non_blocking=True)
+            energy_host.copy_(st.energy[:S], non_blocking=True)
+            # ... and the fresh ones go into their slots; the swap synchronises, which also completes the copies above
+            if take > 0:
+                st.swap_systems(done[:take].astype(np.int32), fresh, stage)
+            else:
+                stream.synchronize()
+            pos_done, energy = pos_host[:m].numpy(), energy_host.numpy()
+            for k, s_ in enumerate(done):
+                sid = int(slot_id[s_])
+                self.results[sid] = {"pos": pos_done[k * n_s:(k + 1) * n_s].copy(), "energy": float(energy[s_]),
+                                     "fire_steps": int(steps[s_]), "status": int(status[s_]), "slot": int(s_)}
+                if status[s_] == ts.TS_FIRE_CONVERGED:
+                    n_done += 1
+                else:
+                    self.failed.append(sid)
+                slot_id[s_] = -1
+            if n_done >= target:
+                return True
+            if take > 0:
+                next_id += take
+                slot_id[done[:take]] = new_ids
+                valid_from[done[:take]] = q + 2              # call q + 1 was enqueued before the swap: its status is stale
+            return not (slot_id >= 0).any()
+
+        try:
+            for r in range(max_rounds):
+                st.fire_step(fp, self.k_check)
+                status_t, steps_t, ev = snaps[r % 2]
+                st.fire_status_async(status_t, steps_t)
+                ev.record(stream)
+                if r > 0 and harvest(r - 1):
+                    break
+            rep = st.poll()
+            if rep.flags:
+                raise ts.TsError(8, "InFlightRelaxer", f"device flags {rep.flags}")
+        finally:
+            self.unfinished = [int(i) for i in slot_id if i >= 0]
+            st.close()
+        return self.results
+
+    def _run_blocking(self, target=None, max_rounds=100000):
         from .state import SimState
         target = self.n_total if target is None else int(target)
         ids = list(range(self.n_slots))

@@ -29,6 +29,23 @@ class _Pot:
         self.c = ts.ts_potential(self.kind, self.n_types, p[0], p[1], p[2], p[3], int(bool(pot.shift_energy)))
 
 
+class PinnedStage:
+    """Page-locked upload buffers for swap_systems, allocated once (cudaHostAlloc is slow) and reused by every swap.
+    A swap synchronises before it returns, so the buffers are free again when the next swap fills them."""
+
+    def __init__(self, torch, tdtype, max_atoms, max_systems):
+        pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory()
+        self.buf = {"pos": pin((max_atoms, 3), tdtype), "vel": pin((max_atoms, 3), tdtype), "mass": pin((max_atoms,), tdtype),
+                    "type": pin((max_atoms,), torch.int32), "cell": pin((max_systems, 3, 3), tdtype),
+                    "uid": pin((max_systems,), torch.int32)}
+
+    def view(self, key, shape):
+        b = self.buf[key]
+        if shape[0] > b.shape[0]:
+            raise ValueError(f"pinned stage too small for {key}: {shape[0]} > {b.shape[0]}")
+        return b[:shape[0]]
+
+
 class SimState:
     """One batch on the device.  `batch` is duck-typed (workloads.Batch): pos, vel, mass, type,
     system_idx, cell, potential, mass_conv, kB, skin, sys_uid."""
@@ -120,6 +137,11 @@ class SimState:
     def converged_mask(self):
         return ts.ts_converged_mask(self.handle, self.S)
 
+    def fire_status_async(self, status, steps):
+        """FIRE status / step counts into pinned int32 host tensors [S], enqueued on the current stream (no sync)."""
+        ts.ts_fire_status_async(self.handle, status.data_ptr() if status is not None else 0,
+                                steps.data_ptr() if steps is not None else 0)
+
     def get_neighbors(self):
         return ts.ts_get_neighbors(self.handle, self.N)
 
@@ -143,27 +165,36 @@ class SimState:
     def launch_count(self):
         return ts.ts_launch_count(self.handle)
 
-    def swap_systems(self, slots, fresh):
-        """Replace the systems in `slots` by those of `fresh` (duck-typed batch, same sizes)."""
-        d, alive = self._upload_fresh(fresh)
+    def swap_systems(self, slots, fresh, stage=None):
+        """Replace the systems in `slots` by those of `fresh` (duck-typed batch, same sizes).  stage: a PinnedStage
+        (page-locked upload buffers): the uploads are then enqueued without blocking on the work already in the stream."""
+        d, alive = self._upload_fresh(fresh, stage)
         ts.ts_swap_systems(self.handle, slots, d)   # synchronises: the uploads may be released afterwards
         del alive
 
-    def _upload_fresh(self, fresh):
+    def pinned_stage(self, max_atoms, max_systems):
+        return PinnedStage(self.torch, self.tdtype, max_atoms, max_systems)
+
+    def _upload_fresh(self, fresh, stage=None):
         """Device copies of a duck-typed batch for a swap / repack and their descriptor (kept alive by the caller)."""
         torch = self.torch
         n = int(np.asarray(fresh.cell).shape[0])
         nat = int(np.asarray(fresh.pos).shape[0])
         dev = self.device
 
-        def up(a, dt, shape):
-            return torch.from_numpy(np.ascontiguousarray(np.asarray(a).reshape(shape))).to(dt).to(dev).contiguous()
+        def up(a, dt, shape, key=None):
+            src = torch.from_numpy(np.ascontiguousarray(np.asarray(a).reshape(shape)))
+            if stage is None:
+                return src.to(dt).to(dev).contiguous()
+            buf = stage.view(key, shape)                   # page-locked, in the device dtype
+            buf.copy_(src)
+            return buf.to(dev, non_blocking=True)
 
         vel = fresh.vel if getattr(fresh, "vel", None) is not None else np.zeros((nat, 3))
-        keep = [up(fresh.pos, self.tdtype, (nat, 3)), up(vel, self.tdtype, (nat, 3)),
-                up(fresh.mass, self.tdtype, (nat,)), up(fresh.type, torch.int32, (nat,)),
-                up(fresh.cell, self.tdtype, (n, 3, 3)),
-                torch.from_numpy(np.asarray(fresh.sys_uid).astype(np.int64)).to(torch.int32).to(dev)]
+        keep = [up(fresh.pos, self.tdtype, (nat, 3), "pos"), up(vel, self.tdtype, (nat, 3), "vel"),
+                up(fresh.mass, self.tdtype, (nat,), "mass"), up(fresh.type, torch.int32, (nat,), "type"),
+                up(fresh.cell, self.tdtype, (n, 3, 3), "cell"),
+                up(np.asarray(fresh.sys_uid).astype(np.int64), torch.int32, (n,), "uid")]
         p = lambda t: C.c_void_p(t.data_ptr())
         d = ts.ts_state_desc(nat, n, self.dtype, self.units, p(keep[0]), p(keep[1]), None, p(keep[2]), p(keep[3]),
                              None, p(keep[4]), None, None, None, p(keep[5]))
