@@ -283,7 +283,10 @@ ts_status ts_set_engine(ts_state *st, int32_t engine);
 
 /* Tell the library that the caller wrote desc.pos / desc.vel from outside (e.g. a host -> device
  * copy): forces are stale and the list must be skin-checked against the new positions before the
- * next step.  Host-side flag only, enqueues nothing.                                              */
+ * next step (the system-resident engine, which keeps its lists from one call to the next in the
+ * pair region of the workspace, builds them anew).  REQUIRED after such a write: without it the
+ * resident engine would go on with lists made for the old positions.  Host-side flag only,
+ * enqueues nothing.                                                                               */
 ts_status ts_invalidate(ts_state *st);
 
 /* Register-only FMA microbenchmark: the ALU peak the roofline of the pair kernels is reported against.

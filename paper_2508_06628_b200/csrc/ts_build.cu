@@ -353,6 +353,9 @@ __global__ void k_force_rebuild(DevState d)
 void launch_build(ts_state *st, bool force, cudaStream_t q)
 {
     const DevState &d = st->d;
+    /* a whole-batch build writes every system's segment of `nbr`: the lists the resident engine saved there are gone
+     * (in mixed mode the kernels below skip the resident engine's systems and their segments stay) */
+    if (!d.mixed) st->res_saved_ok = false;
     if (force) { k_force_rebuild<<<(d.S + 255) / 256, 256, 0, q>>>(d); st->launches += 1; }
     int tb = 256;
     int nba = (int)((d.N + tb - 1) / tb);

@@ -338,6 +338,7 @@ __global__ void k_swap(DevState d, int n, const T *fpos, const T *fvel, const T 
         d.f_nsteps[slot] = 0;
         d.sys_step[slot] = 0ull;
         d.sys_active[slot] = 1;
+        d.res_saved[slot] = 0;                  /* the resident engine's saved list belonged to the system that left */
     }
 }
 

@@ -86,6 +86,8 @@ struct DevState {
     unsigned int *uid_own;       /* [S] persistent ids (copy or iota)  */
     int *sys_engine;             /* [S] 1 = stepped by the system-resident engine (mixed dispatch of a ragged batch) */
     int *res_list;               /* [S] the resident engine's systems, size class after size class */
+    int *res_saved;              /* [S] 1 = the resident engine's list of the system (rows, task words, image table, x_ref / wrap)
+                                  * lies in the system's own segment of `nbr` and matches its stored positions */
     int mixed;                   /* 1: this launch sequence of the general engine skips the systems with sys_engine = 1 */
     /* workspace: per atom */
     void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
@@ -112,6 +114,8 @@ struct ts_state {
     int S_cap;
     bool list_built;             /* a build has been enqueued and no swap since */
     bool forces_current;
+    bool res_saved_ok;           /* nothing has happened since the last resident launch that invalidates res_saved for the
+                                  * whole batch (a general-engine build, positions written from outside, a new plan) */
     bool list_mixed;             /* the general engine's list covers only the systems the resident engine does not step */
     int engine;
     int last_engine;             /* engine that ran the last stepping call */
@@ -126,7 +130,7 @@ struct ts_state {
 struct TsLayout {
     size_t total;
     size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
-        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, res_saved, pos4, spos, xref, cell_count, cell_start, atom_cell,
         atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
 };
 TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);

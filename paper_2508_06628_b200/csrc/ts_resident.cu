@@ -894,6 +894,100 @@ __device__ __noinline__ void build_phase(const ResCfg &rc, uint4 *fr, const unsi
     if (lane == 0 && nnz) atomicAdd(&misc->nnz, nnz);
 }
 
+/* ------------------------------------------------------------------ the list across calls
+ * At the end of a call every CTA copies what it needs to go on without a rebuild -- task words, x_ref | wrap shift of its
+ * own atoms, the image table, and the trips of the rows that are in use -- into its share of the system's own segment
+ * of the general engine's pair array (the resident engine's systems do not use it), and the next call that finds
+ * res_saved[s] = 1 copies it back instead of building the list (a 10-step call of an in-flight FIRE run spends more
+ * than a third of its time in that build).  The flag is 1 only when every CTA of the cluster had room; it is cleared
+ * by the swap kernel for a replaced system and by the host for the whole batch whenever something else wrote the pair
+ * array or the positions (ts_internal.cuh: res_saved_ok).                                                            */
+struct SavedHead { unsigned trips, ntasks, nnz, pad; };
+
+template <typename T>
+__device__ __forceinline__ unsigned char *saved_base(const DevState &d, const ResCfg &rc, int s, int rank, size_t &share)
+{
+    const long long b0 = d.nbr_base[s], b1 = d.nbr_base[s + 1];
+    share = ((size_t)(b1 - b0) * 4u / (size_t)rc.CL) & ~(size_t)15;
+    return (unsigned char *)(d.nbr + b0) + (size_t)rank * share;
+}
+
+/* scan[t] = trips of the tasks before t (scan: ntasks + 1 words of scratch); returns the total */
+__device__ __forceinline__ unsigned trip_scan(const unsigned *tmeta, int ntasks, unsigned *scan)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned run = 0u;
+        for (int t = 0; t < ntasks; ++t) { scan[t] = run; run += tmeta[8 * t] >> 14; }
+        scan[ntasks] = run;
+    }
+    __syncthreads();
+    return scan[ntasks];
+}
+
+/* (plain arguments, no references to the kernel's parameter structs: those would move to local memory) */
+template <typename T>
+__device__ __forceinline__ void save_list(unsigned char *base, size_t share, int *flag, int A, int pitch, int nwarps, int N_s,
+                                       int A_own, const unsigned short *rows, const unsigned *tmeta, const unsigned *gtab,
+                                       const Q4<T> *oref, Q4<T> Rr, unsigned nnz, bool overflow, unsigned *scan)
+{
+    const int ntasks = (A_own + 7) >> 3;
+    const unsigned total = trip_scan(tmeta, ntasks, scan);
+    const size_t o_meta = sizeof(SavedHead), o_ref = o_meta + 4u * (size_t)A, o_gtab = o_ref + sizeof(Q4<T>) * (size_t)A;
+    const size_t o_rows = o_gtab + 4u * (size_t)((N_s + 3) & ~3);
+    if (overflow || o_rows + 256u * (size_t)total > share) {      /* no room (or no list): the next call builds it */
+        if (threadIdx.x == 0) *flag = 0;
+        return;
+    }
+    if (threadIdx.x == 0) {
+        SavedHead h;
+        h.trips = total; h.ntasks = (unsigned)ntasks; h.nnz = nnz; h.pad = 0u;
+        *(SavedHead *)base = h;
+    }
+    unsigned *gm = (unsigned *)(base + o_meta), *gg = (unsigned *)(base + o_gtab);
+    for (int k = threadIdx.x; k < 8 * ntasks; k += blockDim.x) gm[k] = tmeta[k];
+    for (int k = threadIdx.x; k < N_s; k += blockDim.x) gg[k] = gtab[k];
+    if ((int)threadIdx.x < A_own) ((Q4<T> *)(base + o_ref))[threadIdx.x] = sizeof(T) == 4 ? oref[threadIdx.x] : Rr;
+    const int lane = threadIdx.x & 31;
+    for (int t = threadIdx.x >> 5; t < ntasks; t += nwarps) {
+        const uint4 *src = (const uint4 *)(rows + (size_t)t * pitch * 8);
+        uint4 *dst = (uint4 *)(base + o_rows + 256u * (size_t)scan[t]);
+        const int n16 = (int)(scan[t + 1] - scan[t]) * 16;
+        for (int k = lane; k < n16; k += 32) dst[k] = src[k];
+    }
+}
+
+/* the reverse; the own atoms' x_ref | wrap shift go to oref (fp32) or come back in the return value (fp64) */
+template <typename T>
+__device__ __forceinline__ Q4<T> restore_list(const unsigned char *base, int A, int pitch, int nwarps, int N_s, int A_own,
+                                           unsigned short *rows, unsigned *tmeta, unsigned *gtab, Q4<T> *oref,
+                                           ResMisc *misc, unsigned *scan)
+{
+    const int ntasks = (A_own + 7) >> 3;
+    const size_t o_meta = sizeof(SavedHead), o_ref = o_meta + 4u * (size_t)A, o_gtab = o_ref + sizeof(Q4<T>) * (size_t)A;
+    const size_t o_rows = o_gtab + 4u * (size_t)((N_s + 3) & ~3);
+    const unsigned *gm = (const unsigned *)(base + o_meta), *gg = (const unsigned *)(base + o_gtab);
+    for (int k = threadIdx.x; k < 8 * ntasks; k += blockDim.x) tmeta[k] = gm[k];
+    for (int k = threadIdx.x; k < N_s; k += blockDim.x) gtab[k] = gg[k];
+    Q4<T> R;
+    R.a = R.b = R.c = R.d = 0;
+    if ((int)threadIdx.x < A_own) {
+        R = ((const Q4<T> *)(base + o_ref))[threadIdx.x];
+        if (sizeof(T) == 4) oref[threadIdx.x] = R;
+    }
+    if (threadIdx.x == 0) { misc->nnz = ((const SavedHead *)base)->nnz; misc->overflow = 0; }
+    trip_scan(tmeta, ntasks, scan);
+    const int lane = threadIdx.x & 31;
+    for (int t = threadIdx.x >> 5; t < ntasks; t += nwarps) {
+        uint4 *dst = (uint4 *)(rows + (size_t)t * pitch * 8);
+        const uint4 *src = (const uint4 *)(base + o_rows + 256u * (size_t)scan[t]);
+        const int n16 = (int)(scan[t + 1] - scan[t]) * 16;
+        for (int k = lane; k < n16; k += 32) dst[k] = src[k];
+    }
+    __syncthreads();
+    return R;
+}
+
 /* ------------------------------------------------------------------ block / cluster reduction of 8 doubles */
 /* red[warp][0..6] already holds the warp partials of E, W; ke is this thread's kinetic energy.
  * Returns total k to thread k < 8 of cluster rank 0 (fixed summation order: deterministic). */
@@ -1089,11 +1183,41 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         bool have_ev = false;                         /* the last pair pass also produced E (and W) */
         cluster.sync();                               /* constants visible; previous system fully retired everywhere */
 
+        /* the list the last call left for these positions (every CTA of the cluster reads the same flag) */
+        bool restored = false;
+#ifdef TS_RES_TIMING
+        long long rt0 = clock64();
+#endif
+        if (!DUMP && d.res_saved[s]) {
+            size_t share;
+            const unsigned char *sbase = saved_base<T>(d, rc, s, rank, share);
+            const Q4<T> R = restore_list<T>(sbase, rc.A, rc.pitch, rc.nwarps, N_s, A_own, rows, tmeta, gtab, oref, misc, (unsigned *)red);
+            if (own) {
+                /* home slots of all atoms in every CTA, with the wrap shift of the build that made the list */
+                if (!OWN_SMEM) Rr = R;
+                const Q4<T> X = OWN_SMEM ? ox[tid] : Xr;
+                const int wpack = bits_from(R.d);
+                const T wa = (T)(signed char)(wpack & 0xff), wb = (T)(signed char)((wpack >> 8) & 0xff), wc = (T)(signed char)((wpack >> 16) & 0xff);
+                publish_home<T>(cluster, CL, posb, zt, hs, X.a - (wa * gh[0] + wb * gh[3] + wc * gh[6]),
+                                X.b - (wa * gh[1] + wb * gh[4] + wc * gh[7]), X.c - (wa * gh[2] + wb * gh[5] + wc * gh[8]), ty);
+            }
+            if (tid < 8) {
+                const T far = (T)1e15;
+                st_pos(posb, (unsigned)(N8 + tid) * 16u, zt, far, far, far, 0);
+            }
+            cluster.sync();
+            ghost_pass<T>(posb, zt, gtab, gh, N_s);
+            __syncthreads();
+            restored = true;
+        }
+#ifdef TS_RES_TIMING
+        if (tid == 0) atomicAdd(&g_res_prof[12], (unsigned long long)(clock64() - rt0));
+#endif
 #ifdef TS_RES_TIMING
         long long prof_acc[12] = { 0 }, prof_t = clock64();
 #endif
         for (int n = 0; n <= n_steps; ++n) {
-            bool rebuild = n == 0;
+            bool rebuild = n == 0 && !restored;
             const bool last = n == n_steps;
             if (FIRE && n > 0) {
                 if (fsm->nsteps >= fp.max_steps) {     /* reported as failed, never counted (R24) */
@@ -1341,6 +1465,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
             ke = 0.5 * (double)((const T *)d.mass)[gi] * d.mass_conv * ((double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2);
             if (!(fabs((double)f0) + fabs((double)f1) + fabs((double)f2) < 1e300)) atomicOr(&d.status->flags, TS_FLAG_NONFINITE);
         }
+        if (rank == 0 && tid == 0) d.res_saved[s] = 1;   /* a CTA without room for its part clears it after the barrier in reduce8 */
         const double tot = reduce8(cluster, CL, rank, ke, red, cred, rc.nwarps);
         if (rank == 0 && tid < 8) {
             if (tid == 0) d.energy[s] = tot;
@@ -1365,6 +1490,19 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
                     d.sys_active[s] = fsm->status == TS_FIRE_RUNNING ? 1 : 0;
                 }
             }
+        }
+        {
+#ifdef TS_RES_TIMING
+            long long st0 = clock64();
+#endif
+            size_t share;
+            unsigned char *sbase = saved_base<T>(d, rc, s, rank, share);
+            save_list<T>(sbase, share, d.res_saved + s, rc.A, rc.pitch, rc.nwarps, N_s, A_own, rows, tmeta, gtab, oref, Rr, misc->nnz,
+                         misc->overflow != 0, (unsigned *)red);
+#ifdef TS_RES_TIMING
+            __syncthreads();
+            if (tid == 0) atomicAdd(&g_res_prof[13], (unsigned long long)(clock64() - st0));
+#endif
         }
         cluster.sync();                               /* nobody overwrites shared state a peer still reads */
     }
@@ -1579,6 +1717,7 @@ static ResPlan *resident_plan(ts_state *st)
     ResPlan *p = plan_of(st);
     if (p->checked) return p;
     p->checked = true; p->n_classes = 0; p->n_general = st->d.S;
+    st->res_saved_ok = false;                /* a new plan: other launch shapes, the saved lists do not fit them */
     const DevState &d = st->d;
     const int S = d.S;
     free(p->cls_of_sys);
@@ -1658,6 +1797,7 @@ int resident_general_count(ts_state *st) { return resident_plan(st)->n_general; 
 void resident_invalidate(ts_state *st)
 {
     if (st->res_plan) plan_of(st)->checked = false;
+    st->res_saved_ok = false;
 }
 
 /* An equal-size swap brought new cells (HOST copy, [n, 9] in the state dtype) into `slots`: the plan stays when every
@@ -1677,7 +1817,7 @@ void resident_after_swap(ts_state *st, const int32_t *slots, int n, const void *
         const double *h = g.h;
         const double c00 = h[4] * h[8] - h[5] * h[7], c01 = h[5] * h[6] - h[3] * h[8], c02 = h[3] * h[7] - h[4] * h[6];
         const double det = h[0] * c00 + h[1] * c01 + h[2] * c02;
-        if (!(fabs(det) > 0.0)) { p->checked = false; return; }
+        if (!(fabs(det) > 0.0)) { p->checked = false; st->res_saved_ok = false; return; }
         const double id = 1.0 / det;
         const double hinv[9] = { c00 * id, (h[2] * h[7] - h[1] * h[8]) * id, (h[1] * h[5] - h[2] * h[4]) * id,
                                  c01 * id, (h[0] * h[8] - h[2] * h[6]) * id, (h[2] * h[3] - h[0] * h[5]) * id,
@@ -1691,7 +1831,7 @@ void resident_after_swap(ts_state *st, const int32_t *slots, int n, const void *
             const ResCfg &cfg = p->cls[c].cfg;
             fits = (int)ceil(need.nbar * slack) <= cfg.pitch && need.slots <= (double)cfg.NS;
         }
-        if (!fits) { p->checked = false; return; }
+        if (!fits) { p->checked = false; st->res_saved_ok = false; return; }
     }
 }
 
@@ -1746,6 +1886,9 @@ static ts_status launch_classes(ts_state *st, bool fire, const MdConst &c, int n
     if (p->n_classes > 1 && !plan_streams(p)) return TS_ERR_CUDA;
     ResKernel k = pick_kernel(st, fire);
     TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
+    /* saved lists: valid per system (res_saved) unless something invalidated them for the whole batch since the last launch */
+    if (!st->res_saved_ok) TS_CUDA_OK(st, cudaMemsetAsync(st->d.res_saved, 0, sizeof(int) * (size_t)st->d.S, q));
+    st->res_saved_ok = true;
     if (p->n_classes > 1) TS_CUDA_OK(st, cudaEventRecord(p->ev_start, q));
     for (int ci = 0; ci < p->n_classes; ++ci) {
         ResClass &cl = p->cls[ci];
@@ -1825,6 +1968,7 @@ extern "C" ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int
     cfg.dump_cta_bytes = (unsigned)(cta_words * 4);
     cfg.n_clusters = 1;
     st->list_built = false;                                 /* the general engine's list lived there */
+    st->res_saved_ok = false;                               /* and so did the saved lists of the resident engine */
     ResKernel k = st->d.dtype == TS_F32 ? (ResKernel)k_resident_md<float, TS_LJ, false, false, true>
                                         : (ResKernel)k_resident_md<double, TS_LJ, false, false, true>;   /* the build does not depend on the potential */
     if (cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem) != cudaSuccess) {

@@ -337,6 +337,7 @@ extern "C" ts_status ts_invalidate(ts_state *st)
 {
     if (!st) return TS_ERR_INVALID_ARG;
     st->forces_current = false;
+    st->res_saved_ok = false;             /* the resident engine's saved lists were built for other positions */
     return TS_OK;
 }
 

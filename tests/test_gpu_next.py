@@ -175,3 +175,78 @@ def test_external_model_fire_matches_library_fire(ts, orc):
     assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
     assert list(st.converged_mask()[2]) == [60, 60, 60]
     st.close(); ref.close()
+
+
+# ------------------------------------------------------------------ the resident engine's list across calls
+def _chunked_vs_single(ts, b, n, chunk, mode, params):
+    """The same run as one call of n steps and as calls of `chunk` steps; returns the two states and rebuild counts."""
+    out = []
+    for step in (n, chunk):
+        st = ts.SimState(b, engine=1)
+        r0 = st.poll().resident_rebuilds
+        for _ in range(n // step):
+            if mode == "md":
+                st.md_step(params, step)
+            else:
+                st.fire_step(params, step)
+        rep = st.poll()
+        assert rep.flags == 0 and rep.engine == 1
+        out.append((st.numpy("pos").copy(), st.numpy("vel").copy(), st.numpy("energy").copy(), rep.resident_rebuilds - r0))
+        st.close()
+    return out
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_resident_list_survives_calls_md(ts, orc, dtype):
+    """Calls of one step continue with the list the last call saved (no build per call): the trajectory is that of one
+    long call, the number of list builds is the same (one forced build per system in the first call only), and it
+    follows the oracle."""
+    b = wl.cfg2(n_systems=3, reps=4, dtype=dtype)                    # 3 x 256 atoms, LJ, BAOAB, clusters of one CTA
+    md = ts.md_params(**b.md)
+    (p1, v1, e1, rb1), (p2, v2, e2, rb2) = _chunked_vs_single(ts, b, 60, 1, "md", md)
+    # not bitwise: the last step of a call computes its forces together with E (another summation order than the
+    # forces-only pass of the steps before it), and one-step calls take that pass every step
+    tol = 1e-4 if dtype == "f32" else 1e-9
+    assert np.abs(p1 - p2).max() <= tol and np.abs(v1 - v2).max() <= tol
+    assert abs(rb1 - rb2) <= 3 and rb2 < 3 * 20                      # 60 one-step calls did not build 180 lists
+    if dtype == "f64":
+        o = orc.md_run(b, "baoab", b.md["dt"], 60, friction=b.md["friction"], temperature=b.md["temperature"], seed=b.md["seed"])
+        assert np.abs(p2 - o["pos"]).max() <= 1e-8
+
+
+def test_resident_list_survives_calls_cluster_of_two(ts):
+    """The same with systems large enough for a cluster of two CTAs (every CTA saves its own part)."""
+    b = wl.cfg2(n_systems=2, reps=6, dtype="f32")                    # 2 x 864 atoms
+    md = ts.md_params(**b.md)
+    (p1, v1, e1, rb1), (p2, v2, e2, rb2) = _chunked_vs_single(ts, b, 120, 5, "md", md)
+    assert np.abs(p1 - p2).max() <= 1e-4 and np.abs(v1 - v2).max() <= 1e-4 and abs(rb1 - rb2) <= 2 and rb2 < 2 * 24
+
+
+def test_resident_list_survives_calls_fire_and_swap(ts, orc):
+    """FIRE in calls of 5 steps equals FIRE in one call; a swapped-in system gets a fresh build (its slot's saved list
+    belonged to the system that left), an invalidated state rebuilds everything."""
+    b = wl.cfg4(range(4), n_atoms=64)
+    fire = dict(b.fire, f_max=1e-30, max_steps=10 ** 6)
+    (p1, v1, e1, rb1), (p2, v2, e2, rb2) = _chunked_vs_single(ts, b, 60, 5, "fire", fire)
+    assert np.abs(p1 - p2).max() <= 1e-9 and np.abs(v1 - v2).max() <= 1e-9 and abs(rb1 - rb2) <= 2
+    st = ts.SimState(b, engine=1)
+    st.fire_step(fire, 20)
+    st.swap_systems([2], wl.cfg4([9], n_atoms=64))
+    st.fire_step(fire, 20)
+    st.fire_step(fire, 20)
+    pos, off = st.numpy("pos"), st.sys_offset
+    for k, (sid, n) in enumerate([(0, 60), (1, 60), (9, 40), (3, 60)]):
+        one = wl.cfg4([sid], n_atoms=64)
+        o = orc.fire_run(one, dict(one.fire, f_max=1e-30, max_steps=10 ** 6), n)
+        assert np.abs(pos[off[k]:off[k + 1]] - o["pos"]).max() <= 1e-8, sid
+    # positions written from outside + ts_invalidate: the saved lists are dropped, the result is that of a fresh state
+    new_pos = st.pos.clone()
+    new_pos[: int(off[1])] += 0.05
+    st.pos.copy_(new_pos)
+    st.invalidate()
+    st.md_step(ts.md_params(integrator="nve", dt=1e-3), 0, ts.TS_WANT_ENERGY)
+    f1, e1 = st.numpy("force").copy(), st.numpy("energy").copy()
+    o = orc.energy_forces(wl.with_(b, pos=new_pos.cpu().numpy()))      # cfg4 systems share cell, types and masses
+    assert np.abs(f1 - o["F"]).max() <= 1e-9 * max(1.0, np.abs(o["F"]).max())
+    st.close()
+
