@@ -115,9 +115,19 @@ def _check(code, what, handle=None):
         raise TsError(code, what, detail)
 
 
+_raw_stream = None
+
+
 def _stream():
+    """torch's current CUDA stream as a raw handle.  torch.cuda.current_stream() builds a Stream object (~20 us); the
+    raw getter behind it costs about a microsecond, which matters for callers that step once per call."""
+    global _raw_stream
     import torch
-    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if _raw_stream is None:
+        fast = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+        _raw_stream = (lambda: fast(torch.cuda.current_device())) if fast is not None else \
+                      (lambda: torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(_raw_stream())
 
 
 # ------------------------------------------------------------------------------- 1:1 entry points
