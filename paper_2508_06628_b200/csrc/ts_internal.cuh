@@ -51,7 +51,8 @@ struct DevStatus {
     unsigned long long nnz;
     unsigned int list_valid;
     unsigned int pad;
-    unsigned long long res_nnz;       /* resident engine: pairs in the lists at the end of the last call */
+    unsigned long long res_nnz[2];    /* resident engine: pairs in the lists at the end of the last call; two slots used in
+                                       * turn: a call adds into one and clears the other for the next call (no memset launch) */
     unsigned long long res_rebuilds;  /* per-system list builds, summed over systems (both engines)      */
 };
 
@@ -114,6 +115,7 @@ struct ts_state {
     int S_cap;
     bool list_built;             /* a build has been enqueued and no swap since */
     bool forces_current;
+    int res_nnz_slot;            /* slot of DevStatus.res_nnz the last resident launch added into */
     bool res_saved_ok;           /* nothing has happened since the last resident launch that invalidates res_saved for the
                                   * whole batch (a general-engine build, positions written from outside, a new plan) */
     bool list_mixed;             /* the general engine's list covers only the systems the resident engine does not step */

@@ -78,6 +78,7 @@ struct ResCfg {
     int n_clusters;
     unsigned o_pos, o_fr, o_gtab, o_rows, o_fs, o_own, o_meta, o_noise, o_pot, o_red, o_cred, o_misc, o_fire, o_mbar;
     unsigned smem;
+    int nnz_slot;      /* slot of DevStatus.res_nnz this launch adds into (the other one is cleared for the next launch) */
     int noise_helpers; /* the kick buffers of the noise helpers exist (they are left out when they do not fit) */
     float eps_rel;     /* list radius inflation, relative to the longest cell vector */
     const int *syslist; /* device: the systems this launch steps (one size class of the batch); NULL = 0 .. n_list - 1 */
@@ -1098,6 +1099,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
     }
     const int NT = d.n_types;
     for (int k = tid; k < NT * NT; k += blockDim.x) tab[k] = ((const PotEntry<T> *)d.pot)[k];
+    if (blockIdx.x == 0 && tid == 0 && !DUMP) d.status->res_nnz[rc.nnz_slot ^ 1] = 0ull;
     __shared__ unsigned char s_rank[64];          /* image-rank table of the list build */
     if (tid < 64) s_rank[tid] = image_rank8(tid);
 
@@ -1480,7 +1482,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? RES_MAX_THREADS : RES_MAX_THR
         }
         if (tid == 0) {
             if (misc->overflow) atomicOr(&d.status->flags, TS_FLAG_NBR_OVERFLOW);
-            atomicAdd(&d.status->res_nnz, (unsigned long long)misc->nnz);
+            atomicAdd(&d.status->res_nnz[rc.nnz_slot], (unsigned long long)misc->nnz);
             if (rank == 0) {
                 atomicAdd(&d.status->res_rebuilds, (unsigned long long)misc->rebuilds);
                 d.sys_step[s] = step0 + (unsigned long long)(FIRE ? n_done : n_steps);
@@ -1885,7 +1887,7 @@ static ts_status launch_classes(ts_state *st, bool fire, const MdConst &c, int n
     if (p->n_classes < 1) return TS_ERR_UNSUPPORTED;
     if (p->n_classes > 1 && !plan_streams(p)) return TS_ERR_CUDA;
     ResKernel k = pick_kernel(st, fire);
-    TS_CUDA_OK(st, cudaMemsetAsync(&st->d.status->res_nnz, 0, sizeof(unsigned long long), q));
+    st->res_nnz_slot ^= 1;                    /* this call adds into the slot the last call cleared */
     /* saved lists: valid per system (res_saved) unless something invalidated them for the whole batch since the last launch */
     if (!st->res_saved_ok) TS_CUDA_OK(st, cudaMemsetAsync(st->d.res_saved, 0, sizeof(int) * (size_t)st->d.S, q));
     st->res_saved_ok = true;
@@ -1893,6 +1895,7 @@ static ts_status launch_classes(ts_state *st, bool fire, const MdConst &c, int n
     for (int ci = 0; ci < p->n_classes; ++ci) {
         ResClass &cl = p->cls[ci];
         ResCfg cfg = cl.cfg;
+        cfg.nnz_slot = st->res_nnz_slot & 1;
         cudaStream_t sq = ci == 0 ? q : p->aux[ci];
         if (ci > 0) TS_CUDA_OK(st, cudaStreamWaitEvent(sq, p->ev_start, 0));
         cudaLaunchConfig_t lc;

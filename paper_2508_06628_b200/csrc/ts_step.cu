@@ -169,7 +169,8 @@ extern "C" ts_status ts_poll(ts_state *st, ts_report *out, void *stream)
     memset(out, 0, sizeof *out);
     out->flags = hs.flags;
     out->n_rebuilds = (int32_t)hs.n_rebuilds;
-    out->nnz = st->last_engine == 1 ? (int64_t)hs.res_nnz : st->last_engine == 2 ? (int64_t)(hs.res_nnz + hs.nnz) : (int64_t)hs.nnz;
+    const unsigned long long rnnz = hs.res_nnz[st->res_nnz_slot & 1];
+    out->nnz = st->last_engine == 1 ? (int64_t)rnnz : st->last_engine == 2 ? (int64_t)(rnnz + hs.nnz) : (int64_t)hs.nnz;
     out->resident_rebuilds = (int64_t)hs.res_rebuilds;
     out->engine = st->last_engine;
     out->nnz_capacity = st->d.nbr_cap;
