@@ -349,4 +349,8 @@ def test_mixed_engine_dispatch_of_a_ragged_batch(ts, orc):
     st.md_step(dict(b.md), 5)
     o2 = orc.md_run(b, "nve", b.md["dt"], 65)
     assert st.poll().engine == 0 and np.abs(st.numpy("pos") - o2["pos"]).max() <= 1e-8
+    st.set_engine(1)                                 # back: the lists the resident engine had saved are stale and are rebuilt
+    st.md_step(dict(b.md), 5)
+    o3 = orc.md_run(b, "nve", b.md["dt"], 70)
+    assert st.poll().engine == 2 and np.abs(st.numpy("pos") - o3["pos"]).max() <= 1e-8
     st.close()
