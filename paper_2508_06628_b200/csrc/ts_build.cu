@@ -176,6 +176,25 @@ __global__ void k_cellscan(DevState d)
     if (threadIdx.x == 0) {
         d.cell_start[base + nc] = run;
     }
+    /* The ranks k_bin handed out inside a cell came from an atomic counter: their order changes from run to run, and with
+     * it the order of the neighbours in every row and the rounding of every force.  Make them canonical (by atom index):
+     * the block lists the atoms of every cell (nbr_cnt serves as scratch: k_nbr_fill writes it afterwards), then a warp
+     * per cell ranks each atom by the number of smaller indices in its cell. */
+    __syncthreads();
+    const int a0 = d.sysoff[s], a1 = d.sysoff[s + 1];
+    int *order = d.nbr_cnt;
+    for (int i = a0 + threadIdx.x; i < a1; i += blockDim.x) order[d.cell_start[d.atom_cell[i]] + d.atom_rank[i]] = i;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int c = threadIdx.x >> 5; c < nc; c += nw) {
+        const int c0 = d.cell_start[base + c], n = d.cell_start[base + c + 1] - c0;
+        for (int k = lane; k < n; k += 32) {
+            const int id = order[c0 + k];
+            int rank = 0;
+            for (int m = 0; m < n; ++m) rank += order[c0 + m] < id;
+            d.atom_rank[id] = rank;
+        }
+    }
 }
 
 template <typename T>

@@ -76,18 +76,11 @@ __global__ void k_md_pre(DevState d, MdConst c)
     publish_pos<T>(d, i, s, xx[0], xx[1], xx[2]);
 }
 
-/* segmented (per-system) warp reduction + atomicAdd of one double */
-__device__ __forceinline__ void seg_add(double *dst, int s, bool act, double val)
+/* per-system sum of one double in fixed order (ts_sys_sum): dst[s] = sum over the atoms of s; every lane of the warp calls */
+__device__ __forceinline__ void seg_add(const DevState &d, double *dst, int s, bool act, double val)
 {
-    const unsigned FULL = 0xffffffffu;
-    int key = act ? s : -1;
-    int k0 = __shfl_sync(FULL, key, 0);
-    if (__all_sync(FULL, key == k0)) {
-        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(FULL, val, o);
-        if ((threadIdx.x & 31) == 0 && k0 >= 0) atomicAdd(&dst[k0], val);
-    } else if (act) {
-        atomicAdd(&dst[s], val);
-    }
+    const double part[1] = { val };
+    ts_sys_sum<1, 1>(d, act ? s : -1, part, [&](int sl, const double *tot) { dst[sl] = tot[0]; });
 }
 
 template <typename T>
@@ -112,7 +105,7 @@ __global__ void k_md_post(DevState d, MdConst c, int want_ke)
         ke = 0.5 * (double)m * d.mass_conv * ((double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2);
         if (i == d.sysoff[s]) d.sys_step[s] += 1ull;
     }
-    if (want_ke) seg_add(d.kinetic, s, valid, ke);
+    if (want_ke) seg_add(d, d.kinetic, s, valid, ke);
 }
 
 template <typename T>
@@ -131,7 +124,7 @@ __global__ void k_kinetic(DevState d)
         double m = (double)((const T *)d.mass)[i];
         ke = 0.5 * m * d.mass_conv * ((double)v[0] * (double)v[0] + (double)v[1] * (double)v[1] + (double)v[2] * (double)v[2]);
     }
-    seg_add(d.kinetic, s, valid, ke);
+    seg_add(d, d.kinetic, s, valid, ke);
 }
 
 /* ------------------------------------------------------------------ FIRE (O6) */
@@ -239,24 +232,12 @@ __global__ void k_fire_post1(DevState d)
         }
         atomic_max_pos(&d.f_acc[4 * (size_t)s], f2);
     }
-    /* f_acc is [S,4]: stride-4 views for the three sums */
-    const unsigned FULL = 0xffffffffu;
-    int key = act ? s : -1;
-    int k0 = __shfl_sync(FULL, key, 0);
-    if (__all_sync(FULL, key == k0)) {
-        for (int o = 16; o > 0; o >>= 1) {
-            P += __shfl_xor_sync(FULL, P, o);
-            vv += __shfl_xor_sync(FULL, vv, o);
-            f2 += __shfl_xor_sync(FULL, f2, o);
-        }
-        if ((threadIdx.x & 31) == 0 && k0 >= 0) {
-            double *a = d.f_acc + 4 * (size_t)k0;
-            atomicAdd(&a[1], P); atomicAdd(&a[2], vv); atomicAdd(&a[3], f2);
-        }
-    } else if (act) {
-        double *a = d.f_acc + 4 * (size_t)s;
-        atomicAdd(&a[1], P); atomicAdd(&a[2], vv); atomicAdd(&a[3], f2);
-    }
+    /* f_acc is [S,4]: max |F_i|^2 (an atomic max is order-independent), then the three sums in fixed order */
+    const double part[3] = { P, vv, f2 };
+    ts_sys_sum<3, 1>(d, act ? s : -1, part, [&](int sl, const double *tot) {
+        double *a = d.f_acc + 4 * (size_t)sl;
+        a[1] = tot[0]; a[2] = tot[1]; a[3] = tot[2];
+    });
 }
 
 /* (2)..(5) per atom: freeze if converged, else mix (P > 0, with the alpha before its update) or

@@ -89,6 +89,8 @@ struct DevState {
     int *res_list;               /* [S] the resident engine's systems, size class after size class */
     int *res_saved;              /* [S] 1 = the resident engine's list of the system (rows, task words, image table, x_ref / wrap)
                                   * lies in the system's own segment of `nbr` and matches its stored positions */
+    double *red_slots;           /* [(N / 4 + S + 2)][8] partial sums of the general engine's per-system reductions (ts_sys_sum) */
+    int *red_ticket;             /* [S] contributions that have arrived for the system in the running reduction */
     int mixed;                   /* 1: this launch sequence of the general engine skips the systems with sys_engine = 1 */
     /* workspace: per atom */
     void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
@@ -132,7 +134,7 @@ struct ts_state {
 struct TsLayout {
     size_t total;
     size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
-        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, res_saved, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, res_saved, red_slots, red_ticket, pos4, spos, xref, cell_count, cell_start, atom_cell,
         atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
 };
 TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);
@@ -188,6 +190,63 @@ template <> struct Vec4<double> { typedef double4 type; };
 __device__ __forceinline__ int ts_cell_base(const int *sysoff, int s) { return sysoff[s] + s; }
 /* mixed dispatch: the system belongs to the resident engine, the general engine's kernels leave it alone */
 __device__ __forceinline__ bool ts_skip(const DevState &d, int s) { return d.mixed && d.sys_engine[s]; }
+
+/* Per-system sums of the general engine, bitwise reproducible from run to run (fp64 atomics would add in arrival order).
+ * The kernel's threads cover the atoms in order, LANES lanes per atom, so the warps that hold atoms of system s are
+ * w_first(s) .. w_last(s).  Every warp reduces the lanes of each system it holds in a fixed tree and stores the partial in
+ * slot (warp + s) -- a warp that straddles k systems writes k slots, and warp + s is unique and increasing --, then takes a
+ * ticket of the system; the warp that takes the last ticket adds the slots in slot order (lanes stride the slots, fixed
+ * tree) and hands the totals to `fin` (lane 0).  key: system of the lane's atom, -1 for lanes that contribute nothing (all
+ * atoms of a system contribute or none do).  acc: the lane's contribution.                                              */
+template <int NQ, int LANES, typename Fin>
+__device__ __forceinline__ void ts_sys_sum(const DevState &d, int key, const double (&acc)[NQ], Fin fin)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const long long warp = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    unsigned remaining = __ballot_sync(FULL, key >= 0);
+    while (remaining) {
+        const int sl = __shfl_sync(FULL, key, __ffs(remaining) - 1);
+        const bool mine = key == sl;
+        double v[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            v[q] = mine ? acc[q] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(FULL, v[q], o);
+        }
+        const long long w_first = ((long long)d.sysoff[sl] * LANES) >> 5, w_last = ((long long)d.sysoff[sl + 1] * LANES - 1) >> 5;
+        const int expected = (int)(w_last - w_first + 1);
+        int last = 0;
+        if (lane == 0) {
+            double *slot = d.red_slots + 8 * (size_t)(warp + sl);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) __stcg(slot + q, v[q]);
+            __threadfence();
+            last = atomicAdd(&d.red_ticket[sl], 1) == expected - 1;
+        }
+        last = __shfl_sync(FULL, last, 0);
+        if (last) {
+            __threadfence();
+            double tot[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) tot[q] = 0.0;
+            const double *base = d.red_slots + 8 * (size_t)(w_first + sl);
+            for (int k = lane; k < expected; k += 32)
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) tot[q] += __ldcg(base + 8 * (size_t)k + q);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) tot[q] += __shfl_xor_sync(FULL, tot[q], o);
+            if (lane == 0) {
+                fin(sl, tot);
+                d.red_ticket[sl] = 0;                  /* ready for the next reduction (the next kernel in the stream) */
+            }
+        }
+        remaining &= ~__ballot_sync(FULL, mine);
+    }
+}
 
 __device__ __forceinline__ unsigned int ts_pack_nbr(int j, int s0, int s1, int s2)
 {

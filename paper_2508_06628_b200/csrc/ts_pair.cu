@@ -7,8 +7,9 @@
  *
  * Mapping: LPA = 8 lanes per atom read the atom's CSR row in 32-byte pieces (coalesced sector
  * reads), gather x~_j as one float4 / double4 from the pos4 array (L1/L2 resident per system),
- * xor-shuffle over the 8 lanes, then a warp-level segmented reduction of E and W into the fp64
- * per-system outputs (one atomic per warp when the warp sits inside one system).
+ * xor-shuffle over the 8 lanes, then the per-system sums of E and W in fp64 in a fixed order
+ * (ts_sys_sum: one partial per warp and system, added by the warp that arrives last): bitwise
+ * reproducible from run to run, no floating-point atomics.
  */
 #include "ts_internal.cuh"
 #include "ts_pot.cuh"
@@ -97,39 +98,24 @@ __global__ void __launch_bounds__(256, 3) k_pair(DevState d, int masked)
         constexpr int NQ = EV == 2 ? 7 : 1;
         double acc[7] = { 0.5 * (double)e, -0.5 * (double)w0, -0.5 * (double)w1, -0.5 * (double)w2,
                           -0.5 * (double)w3, -0.5 * (double)w4, -0.5 * (double)w5 };
-        int key = act ? s : -1;
-        int sl = __shfl_sync(FULL, key, 0);
-        /* warp inside one system: full warp reduction, one set of atomics */
-        bool whole = __all_sync(FULL, key == sl) && sl >= 0;
-        if (whole) {
+        /* the eight lanes of an atom first (fixed tree), then the per-system sums in fixed order (ts_sys_sum): the
+         * results do not depend on which warp finishes first */
 #pragma unroll
-            for (int q = 0; q < NQ; ++q)
+        for (int q = 0; q < NQ; ++q)
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
-            if ((threadIdx.x & 31) == 0) {
-                atomicAdd(&d.energy[sl], acc[0]);
-                if (EV == 2 && d.virial) {
-                    double *W = d.virial + 9 * (size_t)sl;
-                    atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
-                    atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
-                    atomicAdd(&W[6], acc[3]); atomicAdd(&W[7], acc[5]); atomicAdd(&W[8], acc[6]);
-                }
+            for (int o = 1; o < LPA; o <<= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
+        double part[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) part[q] = sub == 0 ? acc[q] : 0.0;
+        ts_sys_sum<NQ, LPA>(d, act ? s : -1, part, [&](int sl, const double *tot) {
+            d.energy[sl] = tot[0];
+            if (EV == 2 && d.virial) {
+                double *W = d.virial + 9 * (size_t)sl;
+                W[0] = tot[1]; W[1] = tot[2]; W[2] = tot[3];
+                W[3] = tot[2]; W[4] = tot[NQ > 4 ? 4 : 0]; W[5] = tot[NQ > 5 ? 5 : 0];
+                W[6] = tot[3]; W[7] = tot[NQ > 5 ? 5 : 0]; W[8] = tot[NQ > 6 ? 6 : 0];
             }
-        } else {
-#pragma unroll
-            for (int q = 0; q < NQ; ++q)
-#pragma unroll
-                for (int o = 1; o < LPA; o <<= 1) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
-            if (act && sub == 0) {
-                atomicAdd(&d.energy[s], acc[0]);
-                if (EV == 2 && d.virial) {
-                    double *W = d.virial + 9 * (size_t)s;
-                    atomicAdd(&W[0], acc[1]); atomicAdd(&W[1], acc[2]); atomicAdd(&W[2], acc[3]);
-                    atomicAdd(&W[3], acc[2]); atomicAdd(&W[4], acc[4]); atomicAdd(&W[5], acc[5]);
-                    atomicAdd(&W[6], acc[3]); atomicAdd(&W[7], acc[5]); atomicAdd(&W[8], acc[6]);
-                }
-            }
-        }
+        });
     }
 }
 
