@@ -268,6 +268,17 @@ def test_general_engine_is_bitwise_reproducible(ts, dtype):
         out.append(rec)
     for x, y in zip(*out):
         assert np.array_equal(x, y)
+    # the same batch in mixed dispatch (resident engine for the systems it holds, general engine next to it)
+    out = []
+    for _ in range(2):
+        st = ts.SimState(b, engine=1)
+        st.md_step(dict(b.md), 12, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+        st.md_step(dict(b.md), 18, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+        assert st.poll().engine == 2
+        out.append([st.numpy(k).copy() for k in ("pos", "vel", "force", "energy", "virial", "kinetic")])
+        st.close()
+    for x, y in zip(*out):
+        assert np.array_equal(x, y)
     c = wl.cfg4(range(9), n_atoms=96, dtype=dtype if dtype == "f64" else "f32")
     fire = dict(c.fire, f_max=1e-30, max_steps=10 ** 6)
     out = []
