@@ -76,11 +76,11 @@ __global__ void k_md_pre(DevState d, MdConst c)
     publish_pos<T>(d, i, s, xx[0], xx[1], xx[2]);
 }
 
-/* per-system sum of one double in fixed order (ts_sys_sum): dst[s] = sum over the atoms of s; every lane of the warp calls */
-__device__ __forceinline__ void seg_add(const DevState &d, double *dst, int s, bool act, double val)
+/* partial sums of one double per system (ts_sys_store; k_sum_kinetic adds them); every lane of the warp calls */
+__device__ __forceinline__ void seg_store(const DevState &d, int s, bool act, double val)
 {
     const double part[1] = { val };
-    ts_sys_sum<1, 1>(d, act ? s : -1, part, [&](int sl, const double *tot) { dst[sl] = tot[0]; });
+    ts_sys_store<1, 1>(d, act ? s : -1, part);
 }
 
 template <typename T>
@@ -105,7 +105,7 @@ __global__ void k_md_post(DevState d, MdConst c, int want_ke)
         ke = 0.5 * (double)m * d.mass_conv * ((double)v0 * (double)v0 + (double)v1 * (double)v1 + (double)v2 * (double)v2);
         if (i == d.sysoff[s]) d.sys_step[s] += 1ull;
     }
-    if (want_ke) seg_add(d, d.kinetic, s, valid, ke);
+    if (want_ke) seg_store(d, s, valid, ke);
 }
 
 template <typename T>
@@ -124,7 +124,7 @@ __global__ void k_kinetic(DevState d)
         double m = (double)((const T *)d.mass)[i];
         ke = 0.5 * m * d.mass_conv * ((double)v[0] * (double)v[0] + (double)v[1] * (double)v[1] + (double)v[2] * (double)v[2]);
     }
-    seg_add(d, d.kinetic, s, valid, ke);
+    seg_store(d, s, valid, ke);
 }
 
 /* ------------------------------------------------------------------ FIRE (O6) */
@@ -234,10 +234,20 @@ __global__ void k_fire_post1(DevState d)
     }
     /* f_acc is [S,4]: max |F_i|^2 (an atomic max is order-independent), then the three sums in fixed order */
     const double part[3] = { P, vv, f2 };
-    ts_sys_sum<3, 1>(d, act ? s : -1, part, [&](int sl, const double *tot) {
-        double *a = d.f_acc + 4 * (size_t)sl;
+    ts_sys_store<3, 1>(d, act ? s : -1, part);                   /* k_sum_fire adds the slots of every system */
+}
+
+/* P, v.v, F.F of the active systems from the partials of k_fire_post1: one warp per system, slot order */
+__global__ void k_sum_fire(DevState d)
+{
+    const int s = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5);
+    if (s >= d.S || !d.sys_active[s]) return;
+    double tot[3];
+    ts_sys_total<3>(d, s, 1, tot);
+    if ((threadIdx.x & 31) == 0) {
+        double *a = d.f_acc + 4 * (size_t)s;
         a[1] = tot[0]; a[2] = tot[1]; a[3] = tot[2];
-    });
+    }
 }
 
 /* (2)..(5) per atom: freeze if converged, else mix (P > 0, with the alpha before its update) or
@@ -332,16 +342,20 @@ __global__ void k_fire_count(DevState d, int *out /* [2] converged, failed */)
     if (st == TS_FIRE_FAILED) atomicAdd(&out[1], 1);
 }
 
-/* kinetic energies of the systems this engine steps (a memset would wipe those of the resident engine's systems) */
-__global__ void k_zero_kinetic(DevState d)
+/* kinetic energies of the systems this engine steps, from the partials of k_md_post / k_kinetic: one warp per system */
+__global__ void k_sum_kinetic(DevState d)
 {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < d.S && !ts_skip(d, s)) d.kinetic[s] = 0.0;
+    const int s = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5);
+    if (s >= d.S || ts_skip(d, s)) return;
+    double tot[1];
+    ts_sys_total<1>(d, s, 1, tot);
+    if ((threadIdx.x & 31) == 0) d.kinetic[s] = tot[0];
 }
 
 /* ------------------------------------------------------------------ host launchers */
 #define ATOM_GRID(d) (unsigned)(((d).N + 255) / 256), 256
 #define SYS_GRID(d) (unsigned)(((d).S + 127) / 128), 128
+#define SYS_WARP_GRID(d) (unsigned)(((d).S + 3) / 4), 128      /* one warp per system */
 #define BY_DTYPE(st, KERNEL, GRID, ...)                                              \
     do {                                                                             \
         if ((st)->d.dtype == TS_F32) KERNEL<float><<<GRID, 0, q>>>(__VA_ARGS__);     \
@@ -353,14 +367,14 @@ void launch_import(ts_state *st, cudaStream_t q) { BY_DTYPE(st, k_import, ATOM_G
 void launch_md_pre(ts_state *st, const MdConst &c, cudaStream_t q) { BY_DTYPE(st, k_md_pre, ATOM_GRID(st->d), st->d, c); }
 void launch_md_post(ts_state *st, const MdConst &c, bool want_ke, cudaStream_t q)
 {
-    if (want_ke) { k_zero_kinetic<<<SYS_GRID(st->d), 0, q>>>(st->d); st->launches += 1; }
     BY_DTYPE(st, k_md_post, ATOM_GRID(st->d), st->d, c, want_ke ? 1 : 0);
+    if (want_ke) { k_sum_kinetic<<<SYS_WARP_GRID(st->d), 0, q>>>(st->d); st->launches += 1; }
 }
 void launch_kinetic(ts_state *st, cudaStream_t q)
 {
-    k_zero_kinetic<<<SYS_GRID(st->d), 0, q>>>(st->d);
-    st->launches += 1;
     BY_DTYPE(st, k_kinetic, ATOM_GRID(st->d), st->d);
+    k_sum_kinetic<<<SYS_WARP_GRID(st->d), 0, q>>>(st->d);
+    st->launches += 1;
 }
 void launch_fire_init(ts_state *st, const ts_fire_params &p, cudaStream_t q) { BY_DTYPE(st, k_fire_init, ATOM_GRID(st->d), st->d, p); }
 void launch_fire_check0(ts_state *st, const ts_fire_params &p, cudaStream_t q)
@@ -373,6 +387,8 @@ void launch_fire_pre(ts_state *st, const ts_fire_params &p, cudaStream_t q) { BY
 void launch_fire_post(ts_state *st, const ts_fire_params &p, cudaStream_t q)
 {
     BY_DTYPE(st, k_fire_post1, ATOM_GRID(st->d), st->d);
+    k_sum_fire<<<SYS_WARP_GRID(st->d), 0, q>>>(st->d);
+    st->launches += 1;
     BY_DTYPE(st, k_fire_post2, ATOM_GRID(st->d), st->d, p);
     k_fire_sys<<<SYS_GRID(st->d), 0, q>>>(st->d, p);
     st->launches += 1;

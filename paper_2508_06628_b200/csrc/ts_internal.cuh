@@ -89,8 +89,8 @@ struct DevState {
     int *res_list;               /* [S] the resident engine's systems, size class after size class */
     int *res_saved;              /* [S] 1 = the resident engine's list of the system (rows, task words, image table, x_ref / wrap)
                                   * lies in the system's own segment of `nbr` and matches its stored positions */
-    double *red_slots;           /* [(N / 4 + S + 2)][8] partial sums of the general engine's per-system reductions (ts_sys_sum) */
-    int *red_ticket;             /* [S] contributions that have arrived for the system in the running reduction */
+    double *red_slots;           /* [(N / 4 + S + 2)][8] partial sums of the general engine's per-system reductions (ts_sys_store) */
+    int *red_ticket;             /* [S] unused (reserved) */
     int mixed;                   /* 1: this launch sequence of the general engine skips the systems with sys_engine = 1 */
     /* workspace: per atom */
     void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
@@ -191,15 +191,15 @@ __device__ __forceinline__ int ts_cell_base(const int *sysoff, int s) { return s
 /* mixed dispatch: the system belongs to the resident engine, the general engine's kernels leave it alone */
 __device__ __forceinline__ bool ts_skip(const DevState &d, int s) { return d.mixed && d.sys_engine[s]; }
 
-/* Per-system sums of the general engine, bitwise reproducible from run to run (fp64 atomics would add in arrival order).
- * The kernel's threads cover the atoms in order, LANES lanes per atom, so the warps that hold atoms of system s are
- * w_first(s) .. w_last(s).  Every warp reduces the lanes of each system it holds in a fixed tree and stores the partial in
- * slot (warp + s) -- a warp that straddles k systems writes k slots, and warp + s is unique and increasing --, then takes a
- * ticket of the system; the warp that takes the last ticket adds the slots in slot order (lanes stride the slots, fixed
- * tree) and hands the totals to `fin` (lane 0).  key: system of the lane's atom, -1 for lanes that contribute nothing (all
- * atoms of a system contribute or none do).  acc: the lane's contribution.                                              */
-template <int NQ, int LANES, typename Fin>
-__device__ __forceinline__ void ts_sys_sum(const DevState &d, int key, const double (&acc)[NQ], Fin fin)
+/* Per-system sums of the general engine, bitwise reproducible from run to run (fp64 atomics would add in arrival order),
+ * in two kernels and without fences.  The producing kernel's threads cover the atoms in order, LANES lanes per atom, so
+ * the warps that hold atoms of system s are w_first(s) .. w_last(s).  ts_sys_store: every warp reduces the lanes of each
+ * system it holds in a fixed tree and stores the partial in slot (warp + s) of red_slots -- a warp that straddles k
+ * systems writes k slots, and warp + s is unique and increasing.  ts_sys_total (a kernel launched after the producer, one
+ * warp per system): the lanes stride the slots of the system in slot order, then a fixed tree.  key: system of the lane's
+ * atom, -1 for lanes that contribute nothing (all atoms of a system contribute or none do); every lane of the warp calls. */
+template <int NQ, int LANES>
+__device__ __forceinline__ void ts_sys_store(const DevState &d, int key, const double (&acc)[NQ])
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -215,37 +215,32 @@ __device__ __forceinline__ void ts_sys_sum(const DevState &d, int key, const dou
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(FULL, v[q], o);
         }
-        const long long w_first = ((long long)d.sysoff[sl] * LANES) >> 5, w_last = ((long long)d.sysoff[sl + 1] * LANES - 1) >> 5;
-        const int expected = (int)(w_last - w_first + 1);
-        int last = 0;
         if (lane == 0) {
             double *slot = d.red_slots + 8 * (size_t)(warp + sl);
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) __stcg(slot + q, v[q]);
-            __threadfence();
-            last = atomicAdd(&d.red_ticket[sl], 1) == expected - 1;
-        }
-        last = __shfl_sync(FULL, last, 0);
-        if (last) {
-            __threadfence();
-            double tot[NQ];
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) tot[q] = 0.0;
-            const double *base = d.red_slots + 8 * (size_t)(w_first + sl);
-            for (int k = lane; k < expected; k += 32)
-#pragma unroll
-                for (int q = 0; q < NQ; ++q) tot[q] += __ldcg(base + 8 * (size_t)k + q);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q)
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) tot[q] += __shfl_xor_sync(FULL, tot[q], o);
-            if (lane == 0) {
-                fin(sl, tot);
-                d.red_ticket[sl] = 0;                  /* ready for the next reduction (the next kernel in the stream) */
-            }
+            for (int q = 0; q < NQ; ++q) slot[q] = v[q];
         }
         remaining &= ~__ballot_sync(FULL, mine);
     }
+}
+
+/* totals of system s from the slots a kernel with `lanes` lanes per atom stored; the result is in every lane */
+template <int NQ>
+__device__ __forceinline__ void ts_sys_total(const DevState &d, int s, int lanes, double (&tot)[NQ])
+{
+    const int lane = threadIdx.x & 31;
+    const long long w_first = ((long long)d.sysoff[s] * lanes) >> 5, w_last = ((long long)d.sysoff[s + 1] * lanes - 1) >> 5;
+    const int n = (int)(w_last - w_first + 1);
+    const double *base = d.red_slots + 8 * (size_t)(w_first + s);
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) tot[q] = 0.0;
+    for (int k = lane; k < n; k += 32)
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) tot[q] += base[8 * (size_t)k + q];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tot[q] += __shfl_xor_sync(0xffffffffu, tot[q], o);
 }
 
 __device__ __forceinline__ unsigned int ts_pack_nbr(int j, int s0, int s1, int s2)

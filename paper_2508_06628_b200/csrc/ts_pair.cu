@@ -8,8 +8,8 @@
  * Mapping: LPA = 8 lanes per atom read the atom's CSR row in 32-byte pieces (coalesced sector
  * reads), gather x~_j as one float4 / double4 from the pos4 array (L1/L2 resident per system),
  * xor-shuffle over the 8 lanes, then the per-system sums of E and W in fp64 in a fixed order
- * (ts_sys_sum: one partial per warp and system, added by the warp that arrives last): bitwise
- * reproducible from run to run, no floating-point atomics.
+ * (ts_sys_store: one partial per warp and system; k_sum_ev, launched next, adds them in slot
+ * order): bitwise reproducible from run to run, no floating-point atomics.
  */
 #include "ts_internal.cuh"
 #include "ts_pot.cuh"
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256, 3) k_pair(DevState d, int masked)
         constexpr int NQ = EV == 2 ? 7 : 1;
         double acc[7] = { 0.5 * (double)e, -0.5 * (double)w0, -0.5 * (double)w1, -0.5 * (double)w2,
                           -0.5 * (double)w3, -0.5 * (double)w4, -0.5 * (double)w5 };
-        /* the eight lanes of an atom first (fixed tree), then the per-system sums in fixed order (ts_sys_sum): the
+        /* the eight lanes of an atom first (fixed tree), then the per-system partials in fixed order (ts_sys_store): the
          * results do not depend on which warp finishes first */
 #pragma unroll
         for (int q = 0; q < NQ; ++q)
@@ -107,29 +107,34 @@ __global__ void __launch_bounds__(256, 3) k_pair(DevState d, int masked)
         double part[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; ++q) part[q] = sub == 0 ? acc[q] : 0.0;
-        ts_sys_sum<NQ, LPA>(d, act ? s : -1, part, [&](int sl, const double *tot) {
-            d.energy[sl] = tot[0];
-            if (EV == 2 && d.virial) {
-                double *W = d.virial + 9 * (size_t)sl;
-                W[0] = tot[1]; W[1] = tot[2]; W[2] = tot[3];
-                W[3] = tot[2]; W[4] = tot[NQ > 4 ? 4 : 0]; W[5] = tot[NQ > 5 ? 5 : 0];
-                W[6] = tot[3]; W[7] = tot[NQ > 5 ? 5 : 0]; W[8] = tot[NQ > 6 ? 6 : 0];
-            }
-        });
+        ts_sys_store<NQ, LPA>(d, act ? s : -1, part);            /* k_sum_ev adds the slots of every system */
     }
 }
 
-/* zero E / W of the systems whose forces are about to be recomputed */
-__global__ void k_zero_ev(DevState d, int masked, unsigned want)
+/* E / W of the systems k_pair has just evaluated: one warp per system adds the partials k_pair stored, in slot order */
+__global__ void k_sum_ev(DevState d, int masked, unsigned want)
 {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5);
     if (s >= d.S) return;
     if (masked && !d.sys_active[s]) return;
     if (ts_skip(d, s)) return;
     if (d.nbr_len[s] < 0) return;
-    d.energy[s] = 0.0;
-    if ((want & TS_WANT_VIRIAL) && d.virial)
-        for (int k = 0; k < 9; ++k) d.virial[9 * (size_t)s + k] = 0.0;
+    const int lane = threadIdx.x & 31;
+    if ((want & TS_WANT_VIRIAL) && d.virial) {
+        double tot[7];
+        ts_sys_total<7>(d, s, LPA, tot);
+        if (lane == 0) {
+            d.energy[s] = tot[0];
+            double *W = d.virial + 9 * (size_t)s;
+            W[0] = tot[1]; W[1] = tot[2]; W[2] = tot[3];
+            W[3] = tot[2]; W[4] = tot[4]; W[5] = tot[5];
+            W[6] = tot[3]; W[7] = tot[5]; W[8] = tot[6];
+        }
+    } else {
+        double tot[1];
+        ts_sys_total<1>(d, s, LPA, tot);
+        if (lane == 0) d.energy[s] = tot[0];
+    }
 }
 
 template <typename T, int KIND>
@@ -140,9 +145,9 @@ static void launch_pair_k(ts_state *st, unsigned want, bool masked, cudaStream_t
     unsigned nb = (unsigned)((nthreads + 255) / 256);
     if (want) {
         if (!(want & TS_WANT_VIRIAL)) d.virial = nullptr;
-        k_zero_ev<<<(d.S + 127) / 128, 128, 0, q>>>(d, masked ? 1 : 0, want);
         if (d.virial) k_pair<T, KIND, 2><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
         else k_pair<T, KIND, 1><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);
+        k_sum_ev<<<(d.S + 3) / 4, 128, 0, q>>>(d, masked ? 1 : 0, want);
         st->launches += 2;
     } else {
         k_pair<T, KIND, 0><<<nb, 256, 0, q>>>(d, masked ? 1 : 0);

@@ -255,8 +255,8 @@ def test_resident_list_survives_calls_fire_and_swap(ts, orc):
 # ------------------------------------------------------------------ general engine: reproducible reductions
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_general_engine_is_bitwise_reproducible(ts, dtype):
-    """E, W, KE and the FIRE sums of the general engine are added in a fixed order (ts_sys_sum: per-warp partials in slots,
-    summed by the warp that arrives last), not with floating-point atomics: two runs of the same ragged batch -- systems
+    """E, W, KE and the FIRE sums of the general engine are added in a fixed order (ts_sys_store: per-warp partials in
+    slots, added in slot order by a one-warp-per-system kernel), not with floating-point atomics: two runs of the same ragged batch -- systems
     that share warps, systems that span many blocks -- agree bit for bit, trajectories included (FIRE steers by its sums)."""
     b = wl.cfg3(n_systems=12, dtype=dtype, n_range=(32, 1500))
     out = []
