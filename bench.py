@@ -63,8 +63,33 @@ class ClockSampler:
 
     def __init__(self, index):
         self.index, self.proc, self.lines = index, None, []
+        self.nvml, self.samples, self.running = None, [], False
+
+    def _nvml_loop(self):
+        """In-process NVML polling every ~5 ms: the timed region of the default run lasts 80 ms, which one nvidia-smi
+        process (100 ms period) samples once."""
+        n = self.nvml
+        try:
+            h = n.nvmlDeviceGetHandleByIndex(self.index)
+            mx = n.nvmlDeviceGetMaxClockInfo(h, n.NVML_CLOCK_SM)
+            get_reasons = getattr(n, "nvmlDeviceGetCurrentClocksEventReasons", None) or n.nvmlDeviceGetCurrentClocksThrottleReasons
+            bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+            while self.running:
+                sm = n.nvmlDeviceGetClockInfo(h, n.NVML_CLOCK_SM)
+                r = int(get_reasons(h))
+                self.samples.append((float(sm), float(mx), [k for k, b in bits.items() if r & b]))
+                time.sleep(0.005)
+        except Exception:
+            pass
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml, self.running = pynvml, True
+            threading.Thread(target=self._nvml_loop, daemon=True).start()
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "100"],
@@ -78,11 +103,15 @@ class ClockSampler:
             self.lines.append(line.strip())
 
     def stop(self):
-        if not self.proc:
+        self.running = False
+        if not self.proc and not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
         sm, mx, reasons = [], [], set()
+        for a_, b_, r_ in self.samples:
+            sm.append(a_); mx.append(b_); reasons.update(r_)
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ln in self.lines:
             f = [x.strip() for x in ln.split(",")]
@@ -96,7 +125,8 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm),
+                "source": "nvml polled every 5 ms + nvidia-smi every 100 ms" if self.samples else "nvidia-smi every 100 ms"}
 
 
 def rank_system_ids(rank, n_systems):
