@@ -182,7 +182,8 @@ ts_status ts_poll(ts_state *st, ts_report *out, void *stream);
 ts_status ts_converged_mask(ts_state *st, uint8_t *mask, int32_t *status, int32_t *fire_steps,
                             void *stream);
 
-/* The same status words WITHOUT synchronising: status[s] and fire_steps[s] (HOST arrays of S int32, either may be
+/* (InFlightAutobatcher: "after every few steps ... convergence function" -- the check must not stall the device.)
+ * The same status words WITHOUT synchronising: status[s] and fire_steps[s] (HOST arrays of S int32, either may be
  * NULL) are filled by copies enqueued on `stream` behind the work already there; they are valid once the caller has
  * waited for that point of the stream (an event recorded after this call).  The arrays should be page-locked
  * (cudaHostAlloc / a pinned torch tensor): with pageable memory CUDA falls back to a copy that blocks the host.
@@ -239,7 +240,8 @@ ts_status ts_get_resident_neighbors(ts_state *st, int32_t system, int64_t *off, 
 ts_status ts_export_edges(ts_state *st, int64_t *edge_i, int64_t *edge_j, void *edge_shift, int64_t cap,
                           int64_t *n_edges, void *stream);
 
-/* ts_export_edges for callers that must not allocate and cannot lend workspace scratch (code under CUDA graph
+/* (Same operation as ts_export_edges: PAPER.md:56 ModelInterface, :112 graph construction.)
+ * ts_export_edges for callers that must not allocate and cannot lend workspace scratch (code under CUDA graph
  * capture, tight serving loops): same arguments, same result, but the per-system exclusive scan of the edge counts
  * lives in a file-scope device array of the library instead of a workspace region.  No cudaMalloc / cudaFree or
  * allocating library routine is called (no entry point of this library allocates device memory; this one also
