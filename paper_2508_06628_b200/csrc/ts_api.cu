@@ -50,7 +50,6 @@ TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types
     L.res_list = take(4 * (size_t)S);
     L.res_saved = take(4 * (size_t)S);
     L.red_slots = take(64 * ((size_t)N / 4 + (size_t)S + 2));
-    L.red_ticket = take(4 * (size_t)S);
     L.scratch = take(4 * (2 * (size_t)S + 8));
     L.pot = take(sizeof(PotEntry<double>) * (size_t)n_types * n_types);
     L.pos4 = take(4 * w * (size_t)N);
@@ -98,7 +97,7 @@ extern "C" ts_status ts_estimate_system_bytes(int64_t n_atoms, double volume, do
         return TS_ERR_INVALID_ARG;
     size_t w = dtype == TS_F32 ? 4 : 8;
     size_t boundary = (size_t)n_atoms * (3 * 3 * w + w + 4 + 4) + 9 * w + 8 * 11 + 4;
-    size_t per_sys = sizeof(SysGeom) + 9 * w + 8 * 2 + 8 * 2 + 4 * 9 /* incl. sys_rebuild, sys_engine, res_list, res_saved, red_ticket */ + 64 /* red_slots */ + 32 + 8 + 4 + 8 + 4 * 2 /* cell slots */;
+    size_t per_sys = sizeof(SysGeom) + 9 * w + 8 * 2 + 8 * 2 + 4 * 8 /* incl. sys_rebuild, sys_engine, res_list, res_saved */ + 64 /* red_slots */ + 32 + 8 + 4 + 8 + 4 * 2 /* cell slots */;
     size_t ws = (size_t)n_atoms * per_atom_workspace_bytes(dtype) + per_sys +
                 4 * (size_t)ts_system_pair_capacity(n_atoms, volume, r_list, slack);
     *out_bytes = boundary + ws;
@@ -245,7 +244,7 @@ extern "C" ts_status ts_state_create(const ts_state_desc *desc, const ts_potenti
     d.sys_step = (unsigned long long *)(ws + L.sys_step); d.uid_own = (unsigned int *)(ws + L.uid_own);
     d.sys_engine = (int *)(ws + L.sys_engine); d.res_list = (int *)(ws + L.res_list); d.mixed = 0;
     d.res_saved = (int *)(ws + L.res_saved);
-    d.red_slots = (double *)(ws + L.red_slots); d.red_ticket = (int *)(ws + L.red_ticket);
+    d.red_slots = (double *)(ws + L.red_slots);
     d.scratch = (int *)(ws + L.scratch); d.pot = ws + L.pot;
     d.pos4 = ws + L.pos4; d.spos = (double4 *)(ws + L.spos); d.xref = ws + L.xref;
     d.cell_count = (int *)(ws + L.cell_count); d.cell_start = (int *)(ws + L.cell_start);

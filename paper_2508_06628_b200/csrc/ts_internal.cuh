@@ -90,7 +90,6 @@ struct DevState {
     int *res_saved;              /* [S] 1 = the resident engine's list of the system (rows, task words, image table, x_ref / wrap)
                                   * lies in the system's own segment of `nbr` and matches its stored positions */
     double *red_slots;           /* [(N / 4 + S + 2)][8] partial sums of the general engine's per-system reductions (ts_sys_store) */
-    int *red_ticket;             /* [S] unused (reserved) */
     int mixed;                   /* 1: this launch sequence of the general engine skips the systems with sys_engine = 1 */
     /* workspace: per atom */
     void *pos4;                  /* [N] float4 / double4 (x~,y~,z~,type) */
@@ -134,7 +133,7 @@ struct ts_state {
 struct TsLayout {
     size_t total;
     size_t sysoff, geom, hT, nbr_base, nbr_len, f_dt, f_alpha, f_npos, f_nsteps, f_status, f_acc,
-        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, res_saved, red_slots, red_ticket, pos4, spos, xref, cell_count, cell_start, atom_cell,
+        sys_active, sys_rebuild, sys_step, uid_own, sys_engine, res_list, res_saved, red_slots, pos4, spos, xref, cell_count, cell_start, atom_cell,
         atom_rank, atom_wrap, nbr_cnt, nbr_off, nbr, pot, status, scratch;
 };
 TsLayout ts_layout(long long N, int S, long long nbr_cap, int dtype, int n_types);
