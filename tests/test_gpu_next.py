@@ -289,3 +289,49 @@ def test_general_engine_is_bitwise_reproducible(ts, dtype):
         st.close()
     for x, y in zip(*out):
         assert np.array_equal(x, y)
+
+
+# ------------------------------------------------------------------ degenerate systems
+def _degenerate_batch(dtype="f64"):
+    """One atom alone in a big box, two atoms out of each other's reach, a dilute gas whose rows are mostly empty, a
+    crystal, and a single atom in a box so small that it sees its own images: the empty and the self-image corners of
+    the list code, ragged in one batch (argon Lennard-Jones, r_c 8.5, skin 1.0)."""
+    rng = np.random.default_rng(20260511)
+    pot = wl._single_type("lj", wl.LJ_AR["eps"], wl.LJ_AR["sigma"], 0.0, wl.LJ_AR["rc"])
+    m = wl.LJ_AR["mass"]
+
+    def part(pos, L, v_scale=1e-3):
+        pos = np.asarray(pos, dtype=np.float64)
+        vel = rng.normal(0.0, v_scale, size=pos.shape)
+        return (pos, vel, np.full(pos.shape[0], m), np.zeros(pos.shape[0], np.int32), np.eye(3) * L)
+
+    crystal = wl.cfg1(n_systems=1, reps=4, dtype=dtype)                      # 256 atoms, 21 A box
+    parts = [part([[3.0, 4.0, 5.0]], 40.0),
+             part([[1.0, 1.0, 1.0], [21.0, 20.0, 19.0]], 40.0),
+             part(rng.uniform(0.0, 60.0, size=(40, 3)), 60.0),
+             (crystal.pos, crystal.vel, crystal.mass, crystal.type, crystal.cell[0]),
+             part([[0.5, 0.25, 0.125]], 7.0)]                                 # images at 7 A < r_c on every axis
+    md = dict(integrator="nve", dt=2.0, temperature=0.0, friction=0.0, seed=1)
+    return wl._finish("degenerate", parts, pot, wl.MASS_CONV_METAL, wl.KB_METAL, 1.0, dtype, list(range(5)), md=md)
+
+
+@pytest.mark.parametrize("engine", [0, 1])
+def test_degenerate_systems_empty_rows_and_self_images(ts, orc, engine):
+    b = _degenerate_batch()
+    o0 = orc.energy_forces(b)
+    assert o0["E"][0] == 0.0 and o0["E"][1] == 0.0 and o0["E"][4] != 0.0     # nothing in reach / only its own images
+    st = ts.SimState(b, engine=engine)
+    st.md_step(dict(b.md), 0, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == (0 if engine == 0 else 2)        # the 7 A box cannot be resident: mixed dispatch
+    scale = np.maximum(np.abs(o0["E"]), o0["Eabs"]) + 1e-300
+    assert np.all(np.abs(st.numpy("energy") - o0["E"]) <= 1e-12 * scale + 1e-18)
+    assert np.abs(st.numpy("force") - o0["F"]).max() <= 1e-10
+    assert np.abs(st.numpy("virial") - o0["W"]).max() <= 1e-9 * max(1.0, np.abs(o0["W"]).max())
+    for _ in range(3):                                                        # three calls: the lists (also the empty ones) carry over
+        st.md_step(dict(b.md), 10)
+    o = orc.md_run(b, "nve", b.md["dt"], 30)
+    assert st.poll().flags == 0
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8 and np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
+    assert np.allclose(st.numpy("kinetic"), o["KE"], rtol=1e-10, atol=1e-18)
+    st.close()
