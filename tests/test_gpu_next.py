@@ -335,3 +335,40 @@ def test_degenerate_systems_empty_rows_and_self_images(ts, orc, engine):
     assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8 and np.abs(st.numpy("vel") - o["vel"]).max() <= 1e-10
     assert np.allclose(st.numpy("kinetic"), o["KE"], rtol=1e-10, atol=1e-18)
     st.close()
+
+
+@pytest.mark.parametrize("engine", [0, 1])
+def test_degenerate_systems_fire_and_edges(ts, orc, engine):
+    """FIRE on the degenerate batch: the systems without forces converge with 0 steps and stay bit-unchanged, the others
+    follow the oracle; the edge export counts no edge for the empty systems (both export entry points)."""
+    import torch
+    b = _degenerate_batch()
+    fire = dict(dt_start=1.0, dt_max=10.0, f_inc=1.1, f_dec=0.5, alpha_start=0.1, f_alpha=0.99, f_max=1e-6, n_min=5, max_steps=10 ** 6)
+    st = ts.SimState(b, engine=engine)
+    st.fire_step(fire, 40)
+    assert st.poll().flags == 0
+    mask, status, steps = st.converged_mask()
+    assert list(status[:2]) == [ts.TS_FIRE_CONVERGED] * 2 and list(steps[:2]) == [0, 0]        # F = 0 from the start
+    assert status[4] == ts.TS_FIRE_CONVERGED and steps[4] == 0                                # the images' forces cancel
+    off = b.sys_offset
+    assert np.array_equal(st.numpy("pos")[: off[2]], b.pos[: off[2]])
+    o = orc.fire_run(b, fire, 40)
+    assert np.abs(st.numpy("pos") - o["pos"]).max() <= 1e-8
+    assert list(steps) == list(o["state"]["nsteps"]) and list(status) == list(o["state"]["status"])
+    st.close()
+    st = ts.SimState(b, engine=0)
+    st.md_step_external(ts.md_params(**b.md), ts.TS_PHASE_INIT)
+    ei, es = st.export_edges()
+    ei, es = ei.clone(), es.clone()
+    cap = st.capacity()[2]
+    oi = torch.full((2, cap), -7, dtype=torch.int64, device=st.device)
+    os_ = torch.full((cap, 3), -7.0, dtype=st.tdtype, device=st.device)
+    on = torch.full((1,), -7, dtype=torch.int64, device=st.device)
+    st.export_edges_static(oi, os_, on)
+    n = int(on.item())
+    assert n == ei.shape[1] and torch.equal(oi[:, :n], ei) and torch.equal(os_[:n], es)
+    i_sys = st.system_idx[ei[0]].cpu().numpy()
+    counts = np.bincount(i_sys, minlength=5)
+    want = [len(orc.pairs(b.pos[off[s]:off[s + 1]], b.cell[s], b.r_list)[0]) for s in range(5)]
+    assert list(counts) == want and counts[0] == 0 and counts[1] == 0 and counts[4] > 0
+    st.close()
