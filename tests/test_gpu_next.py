@@ -372,3 +372,36 @@ def test_degenerate_systems_fire_and_edges(ts, orc, engine):
     want = [len(orc.pairs(b.pos[off[s]:off[s + 1]], b.cell[s], b.r_list)[0]) for s in range(5)]
     assert list(counts) == want and counts[0] == 0 and counts[1] == 0 and counts[4] > 0
     st.close()
+
+
+def test_largest_resident_system_and_one_beyond(ts, orc):
+    """2048 atoms is the most the resident engine holds (fp32: eight CTAs per system; in fp64 the slots of such a system
+    do not fit shared memory and it goes to the general engine); 2916 atoms always go to the general engine.  fp32 replay
+    parity (R29) after 12 NVE steps in two calls, and the plan says which engine took which."""
+    a = wl.cfg1(n_systems=1, reps=8, dtype="f32", system_ids=[3])            # 8^3 x 4 = 2048 atoms
+    c = wl.cfg1(n_systems=1, reps=9, dtype="f32", system_ids=[4])            # 9^3 x 4 = 2916 atoms
+    b = wl.concat([a, c])
+    st = ts.SimState(b, engine=1)
+    st.md_step(dict(b.md), 5, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    st.md_step(dict(b.md), 7, ts.TS_WANT_ENERGY | ts.TS_WANT_VIRIAL)
+    rep = st.poll()
+    assert rep.flags == 0 and rep.engine == 2
+    bb = wl.with_(b, pos=st.numpy("pos").astype(np.float64), vel=st.numpy("vel").astype(np.float64))
+    o = orc.energy_forces(bb)
+    F = st.numpy("force").astype(np.float64)
+    for s in range(2):
+        a0, a1 = int(b.sys_offset[s]), int(b.sys_offset[s + 1])
+        fmax = np.linalg.norm(o["F"][a0:a1], axis=1).max()
+        bad = np.abs(F[a0:a1] - o["F"][a0:a1]).max(1) > 1e-4 * fmax
+        assert bad.mean() < 0.01                                              # atoms with a pair within rounding of r_c (R29)
+    scale = np.maximum(np.abs(o["E"]), o["Eabs"])
+    assert np.all(np.abs(st.numpy("energy") - o["E"]) <= 1e-5 * scale)
+    off, j, sh = st.get_resident_neighbors(0)                                 # the 2048-atom system is the resident one
+    assert off.shape[0] == 2049 and off[-1] > 0
+    with pytest.raises(ts.TsError):
+        st.get_resident_neighbors(1)                                          # the 2916-atom system is not
+    st.close()
+    d64 = ts.SimState(wl.cfg1(n_systems=1, reps=8, system_ids=[3]), engine=1)   # the same 2048 atoms in fp64
+    d64.md_step(dict(b.md), 2)
+    assert d64.poll().engine == 0
+    d64.close()
